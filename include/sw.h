@@ -1,0 +1,143 @@
+/*
+ * sw.h -- C ABI of libsw.so: Swendsen-Wang multi-cluster sweeps of the 2D q-state
+ * Potts model on one NVIDIA B200 (sm_100a).
+ *
+ * The method (Komura & Okabe, arXiv:1208.2080; line numbers refer to PAPER.md):
+ *   H = -J sum_<ij> delta(S_i, S_j) on an L x L periodic square lattice   PAPER.md:33-38 (eq. 1 up to a constant)
+ *   one sweep =  (1) activate each bond between EQUAL neighbours with p = 1 - exp(-K)
+ *                (2) label the connected components of the active-bond graph
+ *                (3) give every cluster a fresh uniform state in 0..q-1
+ *   the label of a cluster is the smallest site index in it
+ *
+ * Determinism (BASELINE.json north_star; field layout frozen in DESIGN.md, reading R11):
+ *   every draw is Philox4x32-10 with key = (seed lo, seed hi) and counter
+ *   (idx lo, idx hi, sweep t, purpose); purpose 0 = INIT (idx = site), 1 = BOND
+ *   (idx = site >> 1; words 2(site&1), 2(site&1)+1 = right, down bond), 2 = FLIP
+ *   (idx = canonical root).  A bond is active iff draw < T = floor(p * 2^32).
+ *   New state = floor(draw * q / 2^32).  The result of a sweep is therefore a pure
+ *   function of (spins, L, q, K, seed, t) and does not depend on scheduling.
+ *
+ * Conventions
+ *   site i = y*L + x (x fastest); right(i) = y*L + (x+1)%L; down(i) = ((y+1)%L)*L + x.
+ *   spins: uint8, 0..q-1.  labels: uint32 canonical root (minimum site index of the cluster).
+ *   bonds (sw_get_bonds): one byte per site, bit0 = right bond active, bit1 = down bond active.
+ *   All `dst` / `src` / out pointers are HOST memory owned by the caller and sized as annotated;
+ *   device memory is owned by the context (or by the caller of sw_create_ws, who lends it).
+ *   Every call returns a status code; nothing throws or aborts.  Calls on one context must
+ *   not be made concurrently from several threads.
+ *   sw_sweep is asynchronous on the context's CUDA stream; every call that returns data to
+ *   the host synchronises that stream first.
+ */
+#ifndef SW_H
+#define SW_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sw_ctx sw_ctx;   /* opaque; freed only by sw_destroy */
+
+enum {
+    SW_OK = 0,
+    SW_ERR_INVALID_ARG = 1,     /* NULL pointer, L/q/K out of range, spin >= q, ...        */
+    SW_ERR_OOM = 2,             /* device or host allocation failed / workspace too small  */
+    SW_ERR_CUDA = 3,            /* a CUDA runtime call failed (no device, launch error)    */
+    SW_ERR_STATE = 4            /* call not valid in the current state (see each call)     */
+};
+enum { SW_INIT_ORDERED = 0, SW_INIT_RANDOM = 1 };
+
+/* Creation flags (sw_create_ex / sw_create_ws). */
+enum {
+    SW_FLAG_DEFAULT       = 0,
+    SW_FLAG_FORCE_GENERIC = 1,  /* use the any-L reference kernels even where the tiled path applies     */
+    SW_FLAG_LAZY_LABELS   = 2   /* do not materialise canonical labels every sweep; flatten on demand
+                                   (sw_get_labels / sw_measure of cluster sizes).  Same results.        */
+};
+
+/* --- life cycle -------------------------------------------------------------------------------
+ * sw_create: "q-state Potts model ... periodic boundary conditions", one context
+ * per lattice.  2 <= L <= 65536 (L*L <= 2^32 so that a uint32 label can name every site), 2 <= q
+ * <= 255, K = J/k_B T >= 0 or +inf; NaN or negative K -> SW_ERR_INVALID_ARG.  The library
+ * allocates its own device memory on the current device and creates its own stream.            */
+int sw_create(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed);
+int sw_create_ex(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed, uint32_t flags);
+
+/* Device memory and stream lent by the caller (PyTorch in the Python binding).  `dev_ws` must be
+ * a device pointer aligned to 256 bytes with at least sw_workspace_bytes(L, q, flags) bytes and
+ * must outlive the context; `cuda_stream` is a cudaStream_t (NULL = the legacy default stream). */
+size_t sw_workspace_bytes(uint32_t L, uint32_t q, uint32_t flags);
+int sw_create_ws(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed, uint32_t flags,
+                 void *dev_ws, size_t ws_bytes, void *cuda_stream);
+void sw_destroy(sw_ctx *ctx);                      /* NULL is allowed */
+
+/* --- state ------------------------------------------------------------------------------------
+ * sw_init: ORDERED = all spins 0; RANDOM = spin_i = floor(Philox(INIT, i).w0 * q / 2^32).
+ * Sets t = 0 and forgets the labels.  (S_i in 1..q in PAPER.md:35 is stored as 0..q-1.)         */
+int sw_init(sw_ctx *ctx, int mode);
+/* Load a spin configuration and the sweep counter: (spins, t) is the complete state of the
+ * chain, so this is checkpoint/resume.  src: host uint8[L*L], every value < q else
+ * SW_ERR_INVALID_ARG (checked on the device); t <= 2^32 - 1.                                     */
+int sw_set_state(sw_ctx *ctx, const uint8_t *src, uint64_t t);
+
+/* --- the hot path -----------------------------------------------------------------------------
+ * sw_sweep: n full sweeps (PAPER.md:40 steps 1-3), asynchronous on the context stream.
+ * SW_ERR_STATE before sw_init/sw_set_state, or if t + n would pass 2^32 (the sweep field of the
+ * Philox counter is 32 bits).                                                                    */
+int sw_sweep(sw_ctx *ctx, uint64_t n);
+
+/* sw_measure: observables of the current state ("measurement of energy and
+ * magnetization"; cluster statistics from BASELINE.json config 4).  Synchronises.
+ *   energy_bonds    = #{nearest-neighbour pairs with equal spins}, each bond once, 0..2N
+ *                     (E = -J*energy_bonds for H = -J sum delta; eq. 1 subtracts 2N)
+ *   mag_counts[s]   = #{i : spin_i = s}, s = 0..q-1           (host uint64[q])
+ *   n_clusters      = #{clusters} and largest_cluster = max cluster size of the bond
+ *                     configuration drawn in the LAST sweep; both 0 if no sweep since sw_init.
+ * Any out pointer may be NULL ("not wanted"); what is not wanted is not computed.               */
+int sw_measure(sw_ctx *ctx, uint64_t *energy_bonds, uint64_t *mag_counts,
+               uint64_t *n_clusters, uint64_t *largest_cluster);
+
+/* n x (one sweep, one measurement) without a host round trip per sweep; row k of `out`
+ * (host uint64[n][3+q]) = energy_bonds, n_clusters, largest_cluster, mag_counts[0..q-1]
+ * after sweep k.  Synchronises once at the end.                                                  */
+int sw_sweep_measure(sw_ctx *ctx, uint64_t n, uint64_t *out);
+
+/* --- read-back (all synchronise) ---------------------------------------------------------------*/
+int sw_get_spins(sw_ctx *ctx, uint8_t *dst /* host [L*L] */);
+/* canonical roots of the LAST sweep; SW_ERR_STATE if there was none since sw_init */
+int sw_get_labels(sw_ctx *ctx, uint32_t *dst /* host [L*L] */);
+/* bonds of the LAST sweep, one byte per site (bit0 right, bit1 down); SW_ERR_STATE as above      */
+int sw_get_bonds(sw_ctx *ctx, uint8_t *dst /* host [L*L] */);
+/* rows y0 .. y0+nrows-1 only (for sampling a lattice too large to copy whole); what: 0 = spins
+ * (uint8), 1 = labels (uint32), 2 = bonds (uint8)                                                */
+int sw_get_rows(sw_ctx *ctx, int what, uint32_t y0, uint32_t nrows, void *dst);
+int sw_get_threshold(sw_ctx *ctx, uint64_t *T);    /* floor((1-exp(-K)) * 2^32), 0..2^32          */
+int sw_get_time(sw_ctx *ctx, uint64_t *t);         /* sweeps done since sw_init (or set_state's t) */
+int sw_synchronize(sw_ctx *ctx);                   /* wait for the context stream                  */
+
+/* --- introspection ------------------------------------------------------------------------------*/
+typedef struct sw_stats {
+    uint32_t path;              /* 0 = generic kernels, 1 = tiled path                              */
+    uint32_t tile_w, tile_h;    /* tile shape of the tiled path                                     */
+    uint32_t kernels_per_sweep; /* kernel launches one sweep issues                                 */
+    uint64_t kernel_launches;   /* kernels launched by this context so far                          */
+    uint64_t device_bytes;      /* device memory in use by this context                             */
+    uint64_t sweeps;            /* sweeps issued so far                                             */
+} sw_stats;
+int sw_get_stats(sw_ctx *ctx, sw_stats *out);
+/* Time the kernels of the NEXT sweeps individually with CUDA events on the context stream:
+ * after sw_profile_begin, each sw_sweep(n) records per-kernel events; sw_profile_end synchronises
+ * and returns the accumulated milliseconds per kernel slot (see sw_kernel_name).                  */
+#define SW_MAX_KERNEL_SLOTS 8
+int sw_profile_begin(sw_ctx *ctx);
+int sw_profile_end(sw_ctx *ctx, double ms_per_slot[SW_MAX_KERNEL_SLOTS], uint64_t launches_per_slot[SW_MAX_KERNEL_SLOTS]);
+const char *sw_kernel_name(sw_ctx *ctx, int slot); /* NULL if the slot is unused                   */
+const char *sw_last_error(const sw_ctx *ctx);      /* text of the last failure on this context     */
+const char *sw_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

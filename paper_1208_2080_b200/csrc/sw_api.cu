@@ -1,0 +1,497 @@
+// sw_api.cu -- host side of libsw.so: the context, memory plan, launch sequence and the C ABI of
+// include/sw.h.  Every step of the sweep runs in the kernels of sw_tiled.cuh / sw_generic.cuh /
+// sw_observe.cuh; there is no CPU fallback: without a CUDA device every entry point that needs
+// one returns SW_ERR_CUDA.
+#include "../../include/sw.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "sw_common.cuh"
+#include "sw_generic.cuh"
+#include "sw_observe.cuh"
+#include "sw_tiled.cuh"
+
+namespace {
+
+using sw::Params;
+
+enum Slot { SLOT_TILE = 0, SLOT_MERGE = 1, SLOT_FLIP = 2, SLOT_G_BONDS = 3, SLOT_G_INIT = 4,
+            SLOT_G_UNION = 5, SLOT_G_FLATTEN = 6, SLOT_G_FLIP = 7 };
+const char *const kSlotNames[SW_MAX_KERNEL_SLOTS] = {
+    "k_tile_bonds_label", "k_tile_merge", "k_tile_flip", "k_bonds_generic", "k_label_identity",
+    "k_union_generic", "k_flatten_generic", "k_flip_generic"};
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+struct Plan {
+    size_t spins, bonds, labels, border, row, flag, total;   // byte offsets into the workspace
+};
+
+bool tiled_ok(uint32_t L, uint32_t flags) { return (L % sw::kTile == 0) && !(flags & SW_FLAG_FORCE_GENERIC); }
+
+Plan make_plan(uint32_t L, uint32_t q, uint32_t flags)
+{
+    const uint64_t N = (uint64_t)L * L;
+    Plan p{};
+    size_t off = 0;
+    p.spins = off;  off = align_up(off + N);
+    p.bonds = off;  off = align_up(off + ((N + 15) / 16) * 4);
+    p.labels = off; off = align_up(off + N * 4);
+    p.border = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileBorder) : 0));
+    p.row = off;    off = align_up(off + (3 + (size_t)q) * 8);
+    p.flag = off;   off = align_up(off + 4);
+    p.total = off;
+    return p;
+}
+
+}  // namespace
+
+struct sw_ctx {
+    uint32_t L = 0, q = 0, flags = 0;
+    uint64_t N = 0, seed = 0, T = 0, t = 0;
+    double K = 0;
+    bool tiled = false, lazy = false;
+    bool have_spins = false, have_labels = false, labels_flat = false;
+    bool owns_ws = false, owns_stream = false;
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    uint8_t *ws = nullptr;
+    size_t ws_bytes = 0;
+    uint8_t *d_spins = nullptr;
+    uint32_t *d_bonds = nullptr, *d_labels = nullptr, *d_flag = nullptr;
+    sw::TileBorder *d_border = nullptr;
+    unsigned long long *d_row = nullptr;
+    uint32_t *d_sizes = nullptr;          // lazily allocated 4N-byte scratch for cluster sizes
+    uint64_t launches = 0, sweeps = 0;
+    int num_sms = 148;
+    // profiling
+    bool profiling = false;
+    struct Ev { int slot; cudaEvent_t a, b; };
+    std::vector<Ev> events;
+    std::string err;
+};
+
+namespace {
+
+int fail(sw_ctx *c, int code, const char *what)
+{
+    if (c) c->err = what;
+    return code;
+}
+
+int cuda_fail(sw_ctx *c, cudaError_t e, const char *what)
+{
+    if (c) c->err = std::string(what) + ": " + cudaGetErrorString(e);
+    return SW_ERR_CUDA;
+}
+
+#define SW_CUDA(c, call)                                            \
+    do {                                                            \
+        cudaError_t e_ = (call);                                    \
+        if (e_ != cudaSuccess) return cuda_fail((c), e_, #call);    \
+    } while (0)
+
+// north_star: T = floor(p * 2^32), p = 1 - exp(-K), computed once on the host (R10)
+bool host_threshold(double K, uint64_t *T)
+{
+    if (std::isnan(K) || K < 0.0) return false;
+    if (std::isinf(K)) { *T = 1ull << 32; return true; }
+    const double scaled = std::floor(std::ldexp(-std::expm1(-K), 32));
+    *T = scaled <= 0.0 ? 0ull : (scaled >= 4294967296.0 ? (1ull << 32) : (uint64_t)scaled);
+    return true;
+}
+
+Params make_params(const sw_ctx *c, uint64_t t)
+{
+    Params P{};
+    uint32_t k0 = (uint32_t)c->seed, k1 = (uint32_t)(c->seed >> 32);
+    for (int r = 0; r < 10; ++r) {
+        P.rk0[r] = k0; P.rk1[r] = k1;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    P.L = c->L; P.q = c->q; P.t = (uint32_t)t; P.N = c->N;
+    P.thr_any = c->T ? 0xFFFFFFFFu : 0u;
+    P.thr_m1 = c->T ? (uint32_t)(c->T - 1) : 0u;
+    P.log2L = 0xFFFFFFFFu;
+    for (uint32_t b = 0; b < 17; ++b) if ((1u << b) == c->L) P.log2L = b;
+    P.divL_magic = ((1ull << 40) + c->L - 1) / c->L;
+    return P;
+}
+
+int grid_for(const sw_ctx *c, uint64_t items, int threads)
+{
+    const uint64_t want = (items + threads - 1) / threads;
+    const uint64_t cap = (uint64_t)c->num_sms * 16;
+    return (int)(want < 1 ? 1 : (want > cap ? cap : want));
+}
+
+struct Timed {
+    sw_ctx *c; int slot; cudaEvent_t a = nullptr, b = nullptr;
+    Timed(sw_ctx *c_, int slot_) : c(c_), slot(slot_) {
+        c->launches += 1;
+        if (c->profiling && cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess)
+            cudaEventRecord(a, c->stream);
+    }
+    ~Timed() {
+        if (a && b) { cudaEventRecord(b, c->stream); c->events.push_back({slot, a, b}); }
+    }
+};
+
+int sweep_once(sw_ctx *c)
+{
+    const Params P = make_params(c, c->t);
+    if (c->tiled) {
+        const unsigned tiles = (unsigned)(c->N / sw::kTileSites);
+        { Timed tm(c, SLOT_TILE);
+          sw::k_tile_bonds_label<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_border, P); }
+        { Timed tm(c, SLOT_MERGE);
+          sw::k_tile_merge<<<tiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, P); }
+        { Timed tm(c, SLOT_FLIP);
+          sw::k_tile_flip<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_labels, c->d_spins, P, c->lazy ? 0 : 1); }
+        c->labels_flat = !c->lazy;
+    } else {
+        const int th = 256;
+        { Timed tm(c, SLOT_G_BONDS);
+          sw::k_bonds_generic<<<grid_for(c, (c->N + 15) / 16, th), th, 0, c->stream>>>(c->d_spins, c->d_bonds, P); }
+        { Timed tm(c, SLOT_G_INIT);
+          sw::k_label_identity<<<grid_for(c, c->N, th), th, 0, c->stream>>>(c->d_labels, P); }
+        { Timed tm(c, SLOT_G_UNION);
+          sw::k_union_generic<<<grid_for(c, c->N, th), th, 0, c->stream>>>(c->d_bonds, c->d_labels, P); }
+        if (!c->lazy) {
+            Timed tm(c, SLOT_G_FLATTEN);
+            sw::k_flatten_generic<<<grid_for(c, c->N, th), th, 0, c->stream>>>(c->d_labels, P);
+        }
+        { Timed tm(c, SLOT_G_FLIP);
+          sw::k_flip_generic<<<grid_for(c, c->N, th), th, 0, c->stream>>>(c->d_labels, c->d_spins, P); }
+        c->labels_flat = !c->lazy;
+    }
+    c->t += 1;
+    c->sweeps += 1;
+    c->have_labels = true;
+    return SW_OK;
+}
+
+int ensure_flat(sw_ctx *c)
+{
+    if (c->labels_flat) return SW_OK;
+    const Params P = make_params(c, c->t);
+    c->launches += 1;
+    sw::k_flatten_generic<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_labels, P);
+    SW_CUDA(c, cudaGetLastError());
+    c->labels_flat = true;
+    return SW_OK;
+}
+
+// Enqueue the observable kernels for the current state into the device row `row` (zeroed here).
+int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m, bool want_nc, bool want_big)
+{
+    const Params P = make_params(c, c->t);
+    SW_CUDA(c, cudaMemsetAsync(row, 0, (3 + (size_t)c->q) * 8, c->stream));
+    const bool cl = c->have_labels;
+    uint32_t want = (want_e ? 1u : 0u) | (want_m ? 2u : 0u) | ((cl && (want_nc || want_big)) ? 4u : 0u);
+    if (want) {
+        c->launches += 1;
+        if (c->L % 16 == 0)
+            sw::k_observe_vec16<<<grid_for(c, c->N / 16, sw::kObsThreads), sw::kObsThreads, 0, c->stream>>>(c->d_spins, c->d_labels, P, want, row);
+        else
+            sw::k_observe_scalar<<<grid_for(c, c->N, sw::kObsThreads), sw::kObsThreads, 0, c->stream>>>(c->d_spins, c->d_labels, P, want, row);
+    }
+    if (cl && want_big) {
+        if (!c->d_sizes) SW_CUDA(c, cudaMalloc(&c->d_sizes, c->N * 4));
+        SW_CUDA(c, cudaMemsetAsync(c->d_sizes, 0, c->N * 4, c->stream));
+        c->launches += 2;
+        sw::k_cluster_sizes<<<grid_for(c, (c->N + 15) / 16, 256), 256, 0, c->stream>>>(c->d_labels, c->d_sizes, P);
+        sw::k_max_size<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_sizes, P, row);
+    }
+    SW_CUDA(c, cudaGetLastError());
+    return SW_OK;
+}
+
+// a uint32 size counter wraps to 0 only when one cluster holds all 2^32 sites
+void fix_row(const sw_ctx *c, uint64_t *row)
+{
+    if (row[1] == 1) row[2] = c->N;
+}
+
+int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed, uint32_t flags,
+                  void *dev_ws, size_t ws_bytes, void *stream, bool external)
+{
+    if (!out) return SW_ERR_INVALID_ARG;
+    *out = nullptr;
+    uint64_t T = 0;
+    if (L < 2 || L > 65536 || q < 2 || q > 255 || !host_threshold(K, &T)) return SW_ERR_INVALID_ARG;
+    if (flags & ~(uint32_t)(SW_FLAG_FORCE_GENERIC | SW_FLAG_LAZY_LABELS)) return SW_ERR_INVALID_ARG;
+    sw_ctx *c = new (std::nothrow) sw_ctx();
+    if (!c) return SW_ERR_OOM;
+    c->L = L; c->q = q; c->K = K; c->seed = seed; c->T = T; c->flags = flags;
+    c->N = (uint64_t)L * L;
+    c->tiled = tiled_ok(L, flags);
+    c->lazy = (flags & SW_FLAG_LAZY_LABELS) != 0;
+    const Plan plan = make_plan(L, q, flags);
+    cudaError_t e = cudaGetDevice(&c->device);
+    if (e != cudaSuccess) { delete c; return SW_ERR_CUDA; }
+    cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
+    if (external) {
+        if (!dev_ws || ws_bytes < plan.total || ((uintptr_t)dev_ws % kAlign) != 0) { delete c; return dev_ws ? SW_ERR_OOM : SW_ERR_INVALID_ARG; }
+        c->ws = (uint8_t *)dev_ws; c->stream = (cudaStream_t)stream;
+    } else {
+        if (cudaMalloc(&c->ws, plan.total) != cudaSuccess) { cudaGetLastError(); delete c; return SW_ERR_OOM; }
+        c->owns_ws = true;
+        if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) { cudaFree(c->ws); delete c; return SW_ERR_CUDA; }
+        c->owns_stream = true;
+    }
+    c->ws_bytes = plan.total;
+    c->d_spins = c->ws + plan.spins;
+    c->d_bonds = (uint32_t *)(c->ws + plan.bonds);
+    c->d_labels = (uint32_t *)(c->ws + plan.labels);
+    c->d_border = (sw::TileBorder *)(c->ws + plan.border);
+    c->d_row = (unsigned long long *)(c->ws + plan.row);
+    c->d_flag = (uint32_t *)(c->ws + plan.flag);
+    *out = c;
+    return SW_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *sw_version(void) { return "sw-b200 0.1 (sm_100a)"; }
+
+size_t sw_workspace_bytes(uint32_t L, uint32_t q, uint32_t flags)
+{
+    if (L < 2 || L > 65536 || q < 2 || q > 255) return 0;
+    return make_plan(L, q, flags).total;
+}
+
+int sw_create(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed)
+{
+    return create_common(out, L, q, K, seed, SW_FLAG_DEFAULT, nullptr, 0, nullptr, false);
+}
+
+int sw_create_ex(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed, uint32_t flags)
+{
+    return create_common(out, L, q, K, seed, flags, nullptr, 0, nullptr, false);
+}
+
+int sw_create_ws(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed, uint32_t flags,
+                 void *dev_ws, size_t ws_bytes, void *cuda_stream)
+{
+    return create_common(out, L, q, K, seed, flags, dev_ws, ws_bytes, cuda_stream, true);
+}
+
+void sw_destroy(sw_ctx *c)
+{
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    for (auto &ev : c->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+    if (c->d_sizes) cudaFree(c->d_sizes);
+    if (c->owns_ws) cudaFree(c->ws);
+    if (c->owns_stream) cudaStreamDestroy(c->stream);
+    delete c;
+}
+
+int sw_init(sw_ctx *c, int mode)
+{
+    if (!c) return SW_ERR_INVALID_ARG;
+    if (mode == SW_INIT_ORDERED) {
+        SW_CUDA(c, cudaMemsetAsync(c->d_spins, 0, c->N, c->stream));
+    } else if (mode == SW_INIT_RANDOM) {
+        const Params P = make_params(c, 0);
+        c->launches += 1;
+        sw::k_init_random<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_spins, P);
+        SW_CUDA(c, cudaGetLastError());
+    } else return fail(c, SW_ERR_INVALID_ARG, "sw_init: unknown mode");
+    c->t = 0; c->have_spins = true; c->have_labels = false; c->labels_flat = false;
+    return SW_OK;
+}
+
+int sw_set_state(sw_ctx *c, const uint8_t *src, uint64_t t)
+{
+    if (!c || !src || t > 0xFFFFFFFFull) return fail(c, SW_ERR_INVALID_ARG, "sw_set_state: bad argument");
+    SW_CUDA(c, cudaMemcpyAsync(c->d_spins, src, c->N, cudaMemcpyHostToDevice, c->stream));
+    SW_CUDA(c, cudaMemsetAsync(c->d_flag, 0, 4, c->stream));
+    const Params P = make_params(c, 0);
+    c->launches += 1;
+    sw::k_validate_spins<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_spins, P, c->d_flag);
+    uint32_t bad = 0;
+    SW_CUDA(c, cudaMemcpyAsync(&bad, c->d_flag, 4, cudaMemcpyDeviceToHost, c->stream));
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->have_labels = false; c->labels_flat = false;
+    if (bad) { c->have_spins = false; return fail(c, SW_ERR_INVALID_ARG, "sw_set_state: spin value >= q"); }
+    c->t = t; c->have_spins = true;
+    return SW_OK;
+}
+
+int sw_sweep(sw_ctx *c, uint64_t n)
+{
+    if (!c) return SW_ERR_INVALID_ARG;
+    if (!c->have_spins) return fail(c, SW_ERR_STATE, "sw_sweep: no spins (call sw_init or sw_set_state)");
+    if (c->t + n > 0x100000000ull) return fail(c, SW_ERR_STATE, "sw_sweep: sweep counter would pass 2^32");
+    for (uint64_t k = 0; k < n; ++k) {
+        const int rc = sweep_once(c);
+        if (rc != SW_OK) return rc;
+    }
+    SW_CUDA(c, cudaGetLastError());
+    return SW_OK;
+}
+
+int sw_measure(sw_ctx *c, uint64_t *energy_bonds, uint64_t *mag_counts, uint64_t *n_clusters, uint64_t *largest_cluster)
+{
+    if (!c) return SW_ERR_INVALID_ARG;
+    if (!c->have_spins) return fail(c, SW_ERR_STATE, "sw_measure: no spins");
+    const int rc = enqueue_observe(c, c->d_row, energy_bonds != nullptr, mag_counts != nullptr,
+                                   n_clusters != nullptr || largest_cluster != nullptr, largest_cluster != nullptr);
+    if (rc != SW_OK) return rc;
+    std::vector<uint64_t> row(3 + c->q);
+    SW_CUDA(c, cudaMemcpyAsync(row.data(), c->d_row, row.size() * 8, cudaMemcpyDeviceToHost, c->stream));
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    fix_row(c, row.data());
+    if (energy_bonds) *energy_bonds = row[0];
+    if (n_clusters) *n_clusters = c->have_labels ? row[1] : 0;
+    if (largest_cluster) *largest_cluster = c->have_labels ? row[2] : 0;
+    if (mag_counts) for (uint32_t s = 0; s < c->q; ++s) mag_counts[s] = row[3 + s];
+    return SW_OK;
+}
+
+int sw_sweep_measure(sw_ctx *c, uint64_t n, uint64_t *out)
+{
+    if (!c || (!out && n)) return SW_ERR_INVALID_ARG;
+    if (!c->have_spins) return fail(c, SW_ERR_STATE, "sw_sweep_measure: no spins");
+    if (c->t + n > 0x100000000ull) return fail(c, SW_ERR_STATE, "sw_sweep_measure: sweep counter would pass 2^32");
+    if (n == 0) return SW_OK;
+    const size_t stride = 3 + (size_t)c->q;
+    const uint64_t chunk_max = 4096;
+    unsigned long long *d_rows = nullptr;
+    SW_CUDA(c, cudaMalloc(&d_rows, (size_t)(n < chunk_max ? n : chunk_max) * stride * 8));
+    int rc = SW_OK;
+    for (uint64_t done = 0; done < n && rc == SW_OK;) {
+        const uint64_t m = (n - done < chunk_max) ? n - done : chunk_max;
+        for (uint64_t k = 0; k < m && rc == SW_OK; ++k) {
+            rc = sweep_once(c);
+            if (rc == SW_OK) rc = enqueue_observe(c, d_rows + k * stride, true, true, true, true);
+        }
+        if (rc == SW_OK) {
+            cudaError_t e = cudaMemcpyAsync(out + done * stride, d_rows, (size_t)m * stride * 8, cudaMemcpyDeviceToHost, c->stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+            if (e != cudaSuccess) rc = cuda_fail(c, e, "sw_sweep_measure copy");
+        }
+        if (rc == SW_OK) for (uint64_t k = 0; k < m; ++k) fix_row(c, out + (done + k) * stride);
+        done += m;
+    }
+    cudaFree(d_rows);
+    return rc;
+}
+
+int sw_get_rows(sw_ctx *c, int what, uint32_t y0, uint32_t nrows, void *dst)
+{
+    if (!c || !dst || (uint64_t)y0 + nrows > c->L) return fail(c, SW_ERR_INVALID_ARG, "sw_get_rows: bad argument");
+    if (nrows == 0) return SW_OK;
+    const uint64_t first = (uint64_t)y0 * c->L, count = (uint64_t)nrows * c->L;
+    if (what == 0) {
+        if (!c->have_spins) return fail(c, SW_ERR_STATE, "no spins");
+        SW_CUDA(c, cudaMemcpyAsync(dst, c->d_spins + first, count, cudaMemcpyDeviceToHost, c->stream));
+    } else if (what == 1) {
+        if (!c->have_labels) return fail(c, SW_ERR_STATE, "no labels: no sweep since sw_init");
+        const int rc = ensure_flat(c);
+        if (rc != SW_OK) return rc;
+        SW_CUDA(c, cudaMemcpyAsync(dst, c->d_labels + first, count * 4, cudaMemcpyDeviceToHost, c->stream));
+    } else if (what == 2) {
+        if (!c->have_labels) return fail(c, SW_ERR_STATE, "no bonds: no sweep since sw_init");
+        const uint64_t chunk = 64ull << 20;
+        uint8_t *tmp = nullptr;
+        SW_CUDA(c, cudaMalloc(&tmp, (size_t)(count < chunk ? count : chunk)));
+        for (uint64_t done = 0; done < count;) {
+            const uint64_t m = (count - done < chunk) ? count - done : chunk;
+            c->launches += 1;
+            sw::k_expand_bonds<<<grid_for(c, m, 256), 256, 0, c->stream>>>(c->d_bonds, tmp, first + done, m);
+            cudaError_t e = cudaMemcpyAsync((uint8_t *)dst + done, tmp, m, cudaMemcpyDeviceToHost, c->stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+            if (e != cudaSuccess) { cudaFree(tmp); return cuda_fail(c, e, "sw_get_bonds copy"); }
+            done += m;
+        }
+        cudaFree(tmp);
+    } else return fail(c, SW_ERR_INVALID_ARG, "sw_get_rows: unknown array");
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    return SW_OK;
+}
+
+int sw_get_spins(sw_ctx *c, uint8_t *dst) { return c ? sw_get_rows(c, 0, 0, c->L, dst) : SW_ERR_INVALID_ARG; }
+int sw_get_labels(sw_ctx *c, uint32_t *dst) { return c ? sw_get_rows(c, 1, 0, c->L, dst) : SW_ERR_INVALID_ARG; }
+int sw_get_bonds(sw_ctx *c, uint8_t *dst) { return c ? sw_get_rows(c, 2, 0, c->L, dst) : SW_ERR_INVALID_ARG; }
+
+int sw_get_threshold(sw_ctx *c, uint64_t *T)
+{
+    if (!c || !T) return SW_ERR_INVALID_ARG;
+    *T = c->T;
+    return SW_OK;
+}
+
+int sw_get_time(sw_ctx *c, uint64_t *t)
+{
+    if (!c || !t) return SW_ERR_INVALID_ARG;
+    *t = c->t;
+    return SW_OK;
+}
+
+int sw_synchronize(sw_ctx *c)
+{
+    if (!c) return SW_ERR_INVALID_ARG;
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    SW_CUDA(c, cudaGetLastError());
+    return SW_OK;
+}
+
+int sw_get_stats(sw_ctx *c, sw_stats *out)
+{
+    if (!c || !out) return SW_ERR_INVALID_ARG;
+    out->path = c->tiled ? 1u : 0u;
+    out->tile_w = out->tile_h = c->tiled ? sw::kTile : 0u;
+    out->kernels_per_sweep = c->tiled ? 3u : (c->lazy ? 4u : 5u);
+    out->kernel_launches = c->launches;
+    out->device_bytes = c->ws_bytes + (c->d_sizes ? c->N * 4 : 0);
+    out->sweeps = c->sweeps;
+    return SW_OK;
+}
+
+int sw_profile_begin(sw_ctx *c)
+{
+    if (!c) return SW_ERR_INVALID_ARG;
+    for (auto &ev : c->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+    c->events.clear();
+    c->profiling = true;
+    return SW_OK;
+}
+
+int sw_profile_end(sw_ctx *c, double ms_per_slot[SW_MAX_KERNEL_SLOTS], uint64_t launches_per_slot[SW_MAX_KERNEL_SLOTS])
+{
+    if (!c || !ms_per_slot || !launches_per_slot) return SW_ERR_INVALID_ARG;
+    c->profiling = false;
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int s = 0; s < SW_MAX_KERNEL_SLOTS; ++s) { ms_per_slot[s] = 0.0; launches_per_slot[s] = 0; }
+    for (auto &ev : c->events) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, ev.a, ev.b) == cudaSuccess) { ms_per_slot[ev.slot] += ms; launches_per_slot[ev.slot] += 1; }
+        cudaEventDestroy(ev.a); cudaEventDestroy(ev.b);
+    }
+    c->events.clear();
+    return SW_OK;
+}
+
+const char *sw_kernel_name(sw_ctx *c, int slot)
+{
+    if (!c || slot < 0 || slot >= SW_MAX_KERNEL_SLOTS) return nullptr;
+    const bool tiled_slot = slot <= SLOT_FLIP;
+    if (tiled_slot != c->tiled) return nullptr;
+    if (slot == SLOT_G_FLATTEN && c->lazy) return nullptr;
+    return kSlotNames[slot];
+}
+
+const char *sw_last_error(const sw_ctx *c) { return c ? c->err.c_str() : "null context"; }
+
+}  // extern "C"

@@ -1,0 +1,93 @@
+// sw_common.cuh -- device-side building blocks shared by the kernels of libsw.so.
+//
+// Philox4x32-10 (Salmon et al., SC'11) with the ten round keys precomputed on the host,
+// the draw layout of include/sw.h (reading R11), and the lock-free union-find
+// primitives on a uint32 parent array (canonical root = minimum index).
+//
+// Product code: shares nothing with oracle/.
+#pragma once
+
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace sw {
+
+constexpr uint32_t kPurposeInit = 0u, kPurposeBond = 1u, kPurposeFlip = 2u;
+
+// Kernel-parameter block: lives in the constant bank, so the round keys cost no registers.
+struct Params {
+    uint32_t rk0[10];     // k0 + r * 0x9E3779B9
+    uint32_t rk1[10];     // k1 + r * 0xBB67AE85
+    uint32_t L;           // linear size
+    uint32_t q;           // number of Potts states
+    uint32_t t;           // sweep counter (Philox counter word 2)
+    uint32_t thr_m1;      // T - 1 (valid when thr_any != 0): bond active iff draw <= thr_m1
+    uint32_t thr_any;     // 0 if T == 0 (no bond can be active), else 0xFFFFFFFF
+    uint32_t log2L;       // log2(L) if L is a power of two, else 0xFFFFFFFF
+    uint64_t N;           // L * L (up to 2^32)
+    uint64_t divL_magic;  // ceil(2^40 / L): (d * magic) >> 40 == d / L for d < 2^24 (L <= 2^16)
+};
+
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               const Params &P)
+{
+    constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
+        const uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+        c0 = hi1 ^ c1 ^ P.rk0[r];
+        c1 = lo1;
+        c2 = hi0 ^ c3 ^ P.rk1[r];
+        c3 = lo0;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// floor(w * q / 2^32): the draw -> state map (R9)
+__device__ __forceinline__ uint32_t state_from_draw(uint32_t w, uint32_t q) { return __umulhi(w, q); }
+
+__device__ __forceinline__ uint32_t flip_state(uint32_t root, const Params &P)
+{
+    return state_from_draw(philox4x32_10(root, 0u, P.t, kPurposeFlip, P).x, P.q);
+}
+
+// ---- union-find on global memory -------------------------------------------------------------
+// labels[] is a forest whose links always point to a smaller index.  Loads bypass L1 (other
+// SMs update the array concurrently); a stale value is still an ancestor, so chases stay valid.
+
+__device__ __forceinline__ uint32_t ld_label(const uint32_t *labels, uint32_t i)
+{
+    return __ldcg(labels + i);
+}
+
+__device__ __forceinline__ uint32_t find_root(const uint32_t *labels, uint32_t a)
+{
+    uint32_t p = ld_label(labels, a);
+    while (p != a) { a = p; p = ld_label(labels, a); }
+    return a;
+}
+
+// Join the sets of a and b.  The larger root is hooked under the smaller with atomicMin; if the
+// word we hit was no longer a root, the link it held is not lost: we carry on uniting its old
+// target with b.  One pass over all bonds yields the complete partition (no outer iteration).
+__device__ __forceinline__ void unite(uint32_t *labels, uint32_t a, uint32_t b)
+{
+    while (true) {
+        a = find_root(labels, a);
+        b = find_root(labels, b);
+        if (a == b) return;
+        if (a < b) { const uint32_t s = a; a = b; b = s; }
+        const uint32_t old = atomicMin(labels + a, b);
+        if (old == a) return;
+        a = old;
+    }
+}
+
+// d / L for d < 64 * L <= 2^22
+__device__ __forceinline__ uint32_t div_L(uint32_t d, const Params &P)
+{
+    return (P.log2L != 0xFFFFFFFFu) ? (d >> P.log2L) : (uint32_t)(((uint64_t)d * P.divL_magic) >> 40);
+}
+
+}  // namespace sw

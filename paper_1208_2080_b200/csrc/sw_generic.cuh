@@ -1,0 +1,124 @@
+// sw_generic.cuh -- reference kernels that work for ANY lattice size 2 <= L <= 65536 (odd,
+// tiny, not a multiple of the tile): one global union-find over all active bonds.  They are the
+// slow-but-general path of libsw.so (and its internal cross-check for the tiled path); the hot
+// path for L % 64 == 0 is in sw_tiled.cuh.
+//
+// Bond storage on the device (both paths): word w of `bonds` covers the 16 consecutive linear
+// sites 16w .. 16w+15; bit j = right bond of site 16w+j, bit 16+j = its down bond.
+#pragma once
+
+#include "sw_common.cuh"
+
+namespace sw {
+
+// --- init / state -------------------------------------------------------------------------------
+
+__global__ void k_init_random(uint8_t *__restrict__ spins, Params P)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += stride) {
+        const uint4 w = philox4x32_10((uint32_t)i, (uint32_t)(i >> 32), 0u, kPurposeInit, P);
+        spins[i] = (uint8_t)state_from_draw(w.x, P.q);
+    }
+}
+
+// flag[0] |= 1 if any spin >= q
+__global__ void k_validate_spins(const uint8_t *__restrict__ spins, Params P, uint32_t *flag)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    bool bad = false;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += stride)
+        bad |= spins[i] >= P.q;
+    if (__any_sync(0xFFFFFFFFu, bad) && (threadIdx.x & 31) == 0) atomicOr(flag, 1u);
+}
+
+// --- step (1): bonds, one thread per 16-site word -----------------------------------------------
+
+__global__ void k_bonds_generic(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds, Params P)
+{
+    const uint64_t n_words = (P.N + 15) >> 4;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    const uint64_t L = P.L;
+    for (uint64_t w = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; w < n_words; w += stride) {
+        uint32_t word = 0;
+        for (uint32_t j = 0; j < 16; ++j) {
+            const uint64_t i = (w << 4) + j;
+            if (i >= P.N) break;
+            const uint64_t y = i / L, x = i - y * L;
+            const uint64_t ir = y * L + (x + 1 == L ? 0 : x + 1);
+            const uint64_t id = (y + 1 == L ? 0 : y + 1) * L + x;
+            const uint8_t s = spins[i];
+            const bool er = s == spins[ir], ed = s == spins[id];
+            if (er | ed) {
+                const uint64_t pair = i >> 1;
+                const uint4 d = philox4x32_10((uint32_t)pair, (uint32_t)(pair >> 32), P.t, kPurposeBond, P);
+                const uint32_t dr = (i & 1) ? d.z : d.x;
+                const uint32_t dd = (i & 1) ? d.w : d.y;
+                if (er && P.thr_any && dr <= P.thr_m1) word |= 1u << j;
+                if (ed && P.thr_any && dd <= P.thr_m1) word |= 1u << (16 + j);
+            }
+        }
+        bonds[w] = word;
+    }
+}
+
+// --- step (2): labels ---------------------------------------------------------------------------
+
+__global__ void k_label_identity(uint32_t *__restrict__ labels, Params P)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += stride)
+        labels[i] = (uint32_t)i;
+}
+
+__global__ void k_union_generic(const uint32_t *__restrict__ bonds, uint32_t *labels, Params P)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    const uint64_t L = P.L;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += stride) {
+        const uint32_t word = bonds[i >> 4];
+        const uint32_t j = (uint32_t)(i & 15);
+        const bool br = (word >> j) & 1u, bd = (word >> (16 + j)) & 1u;
+        if (!(br | bd)) continue;
+        const uint64_t y = i / L, x = i - y * L;
+        if (br) unite(labels, (uint32_t)i, (uint32_t)(y * L + (x + 1 == L ? 0 : x + 1)));
+        if (bd) unite(labels, (uint32_t)i, (uint32_t)((y + 1 == L ? 0 : y + 1) * L + x));
+    }
+}
+
+// labels[i] <- root(i).  In-place is safe: whatever another thread reads is an ancestor.
+__global__ void k_flatten_generic(uint32_t *labels, Params P)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += stride) {
+        const uint32_t l = ld_label(labels, (uint32_t)i);
+        if (l == (uint32_t)i) continue;
+        const uint32_t r = find_root(labels, l);
+        if (r != l) labels[i] = r;
+    }
+}
+
+// --- step (3): flip; works on a flattened OR an unflattened forest ------------------------------
+
+__global__ void k_flip_generic(const uint32_t *__restrict__ labels, uint8_t *__restrict__ spins, Params P)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += stride)
+        spins[i] = (uint8_t)flip_state(find_root(labels, (uint32_t)i), P);
+}
+
+// --- expand the packed bond words to one byte per site (sw_get_bonds) ---------------------------
+
+__global__ void k_expand_bonds(const uint32_t *__restrict__ bonds, uint8_t *__restrict__ out,
+                               uint64_t first_site, uint64_t n_sites)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n_sites; k += stride) {
+        const uint64_t i = first_site + k;
+        const uint32_t word = bonds[i >> 4];
+        const uint32_t j = (uint32_t)(i & 15);
+        out[k] = (uint8_t)(((word >> j) & 1u) | (((word >> (16 + j)) & 1u) << 1));
+    }
+}
+
+}  // namespace sw

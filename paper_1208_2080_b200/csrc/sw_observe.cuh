@@ -1,0 +1,166 @@
+// sw_observe.cuh -- observables of the current state ("measurement of energy and
+// magnetization"; cluster statistics per BASELINE.json config 4).  Runs only on sw_measure /
+// sw_sweep_measure.  All accumulators are 64-bit: energy_bonds can reach 2^33 at L = 65536.
+//
+// Result row layout (device uint64): [0] energy_bonds, [1] n_clusters, [2] largest_cluster,
+// [3 .. 3+q) mag_counts.
+#pragma once
+
+#include "sw_common.cuh"
+
+namespace sw {
+
+constexpr int kObsThreads = 256;
+
+__device__ __forceinline__ void block_add_u64(unsigned long long v, unsigned long long *dst, unsigned long long *s_scratch)
+{
+    // warp shuffle reduce, then one atomic per block
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane == 0) s_scratch[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+        v = (lane < (blockDim.x >> 5)) ? s_scratch[lane] : 0ull;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+        if (lane == 0 && v) atomicAdd(dst, v);
+    }
+}
+
+// Scalar version: any L.  want: bit0 energy, bit1 magnetisation, bit2 n_clusters.
+__global__ void __launch_bounds__(kObsThreads)
+k_observe_scalar(const uint8_t *__restrict__ spins, const uint32_t *__restrict__ labels, Params P,
+                 uint32_t want, unsigned long long *row)
+{
+    __shared__ unsigned int s_hist[256];
+    __shared__ unsigned long long s_scratch[kObsThreads / 32];
+    for (int k = threadIdx.x; k < 256; k += blockDim.x) s_hist[k] = 0;
+    __syncthreads();
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    const uint64_t L = P.L;
+    unsigned long long e = 0, roots = 0;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += stride) {
+        const uint8_t s = spins[i];
+        if (want & 1u) {
+            const uint64_t y = i / L, x = i - y * L;
+            e += (s == spins[y * L + (x + 1 == L ? 0 : x + 1)]);
+            e += (s == spins[(y + 1 == L ? 0 : y + 1) * L + x]);
+        }
+        if (want & 2u) atomicAdd(&s_hist[s], 1u);
+        if (want & 4u) roots += (labels[i] == (uint32_t)i);
+    }
+    __syncthreads();
+    if (want & 2u)
+        for (int k = threadIdx.x; k < (int)P.q; k += blockDim.x)
+            if (s_hist[k]) atomicAdd(row + 3 + k, (unsigned long long)s_hist[k]);
+    if (want & 1u) block_add_u64(e, row + 0, s_scratch);
+    if (want & 4u) block_add_u64(roots, row + 1, s_scratch);
+}
+
+// Vector version: L % 16 == 0; one thread per 16 consecutive sites of a row.
+__global__ void __launch_bounds__(kObsThreads)
+k_observe_vec16(const uint8_t *__restrict__ spins, const uint32_t *__restrict__ labels, Params P,
+                uint32_t want, unsigned long long *row)
+{
+    __shared__ unsigned int s_hist[256];
+    __shared__ unsigned long long s_scratch[kObsThreads / 32];
+    for (int k = threadIdx.x; k < 256; k += blockDim.x) s_hist[k] = 0;
+    __syncthreads();
+    const uint64_t n_groups = P.N >> 4;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    const uint32_t L = P.L, gpr = L >> 4;                  // groups per row
+    unsigned long long e = 0, roots = 0;
+    unsigned int cnt[4] = {0, 0, 0, 0};                    // q <= 4 fast path
+    for (uint64_t g = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; g < n_groups; g += stride) {
+        const uint32_t y = (uint32_t)(g / gpr), gx = (uint32_t)(g - (uint64_t)y * gpr);
+        const uint64_t base = (uint64_t)y * L + ((uint64_t)gx << 4);
+        const uint4 s = *reinterpret_cast<const uint4 *>(spins + base);
+        const uint32_t w[4] = {s.x, s.y, s.z, s.w};
+        if (want & 1u) {
+            const uint32_t next = spins[(uint64_t)y * L + ((gx + 1 == gpr) ? 0u : ((gx + 1) << 4))];
+            const uint32_t yd = (y + 1 == L) ? 0u : y + 1;
+            const uint4 d = *reinterpret_cast<const uint4 *>(spins + (uint64_t)yd * L + ((uint64_t)gx << 4));
+            const uint32_t dw[4] = {d.x, d.y, d.z, d.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const uint32_t hi = (k < 3) ? w[k + 1] : next;
+                const uint32_t r = __funnelshift_r(w[k], hi, 8);             // the right neighbours of the 4 bytes
+                e += (__popc(__vcmpeq4(w[k], r)) + __popc(__vcmpeq4(w[k], dw[k]))) >> 3;
+            }
+        }
+        if (want & 2u) {
+            if (P.q <= 4) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+#pragma unroll
+                    for (uint32_t a = 0; a < 4; ++a)
+                        cnt[a] += __popc(__vcmpeq4(w[k], a * 0x01010101u)) >> 3;
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    atomicAdd(&s_hist[w[k] & 0xFF], 1u);
+                    atomicAdd(&s_hist[(w[k] >> 8) & 0xFF], 1u);
+                    atomicAdd(&s_hist[(w[k] >> 16) & 0xFF], 1u);
+                    atomicAdd(&s_hist[w[k] >> 24], 1u);
+                }
+            }
+        }
+        if (want & 4u) {
+            const uint4 *lp = reinterpret_cast<const uint4 *>(labels + base);
+            const uint32_t i0 = (uint32_t)base;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const uint4 l = lp[k];
+                roots += (l.x == i0 + 4 * k) + (l.y == i0 + 4 * k + 1) + (l.z == i0 + 4 * k + 2) + (l.w == i0 + 4 * k + 3);
+            }
+        }
+    }
+    if ((want & 2u) && P.q <= 4) {
+#pragma unroll
+        for (uint32_t a = 0; a < 4; ++a) if (cnt[a]) atomicAdd(&s_hist[a], cnt[a]);
+    }
+    __syncthreads();
+    if (want & 2u)
+        for (int k = threadIdx.x; k < (int)P.q; k += blockDim.x)
+            if (s_hist[k]) atomicAdd(row + 3 + k, (unsigned long long)s_hist[k]);
+    if (want & 1u) block_add_u64(e, row + 0, s_scratch);
+    if (want & 4u) block_add_u64(roots, row + 1, s_scratch);
+}
+
+// sizes[root(i)] += 1, with run-length aggregation over consecutive sites (clusters are spatially
+// coherent, so a thread's 16 sites usually share one or two roots).  Works on a forest too.
+__global__ void k_cluster_sizes(const uint32_t *__restrict__ labels, uint32_t *sizes, Params P)
+{
+    const uint64_t n_groups = (P.N + 15) >> 4;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t g = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; g < n_groups; g += stride) {
+        uint32_t cur = 0, run = 0;
+        for (uint32_t j = 0; j < 16; ++j) {
+            const uint64_t i = (g << 4) + j;
+            if (i >= P.N) break;
+            uint32_t l = labels[i];
+            if (l != (uint32_t)i) l = find_root(labels, l);
+            if (run && l == cur) { ++run; continue; }
+            if (run) atomicAdd(sizes + cur, run);
+            cur = l; run = 1;
+        }
+        if (run) atomicAdd(sizes + cur, run);
+    }
+}
+
+// row[2] = max over roots of sizes[]; only roots (labels[i] == i) hold a count
+__global__ void k_max_size(const uint32_t *__restrict__ sizes, Params P, unsigned long long *row)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    uint32_t m = 0;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += stride)
+        m = max(m, sizes[i]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(row + 2, (unsigned long long)m);
+}
+
+}  // namespace sw

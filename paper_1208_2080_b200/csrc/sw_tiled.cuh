@@ -1,0 +1,308 @@
+// sw_tiled.cuh -- the hot path of libsw.so for L % 64 == 0: three kernels per sweep.
+//
+//   k_tile_bonds_label  step (1) + tile-local part of step (2)   ("done independently on each site")
+//   k_tile_merge        union-find over the bonds that cross a tile border (PAPER.md:66-68 uses the
+//                       same boundary-only idea one level up, between GPUs)
+//   k_tile_flip         pointer-jumping flatten to the canonical root ("tracks back
+//                       the label variable until [it] remains unchanged") fused with step (3)
+//
+// A tile is 64 x 64 sites; a CTA of 256 threads owns one tile; thread (y = tid/4, c = tid%4) owns
+// the 16 consecutive sites x = 16c .. 16c+15 of tile row y: one 16-byte spin load, one Philox call
+// per site pair, one 32-bit bond word, four 16-byte label stores.
+#pragma once
+
+#include "sw_common.cuh"
+
+namespace sw {
+
+constexpr uint32_t kTile = 64;                       // tile edge
+constexpr uint32_t kTileSites = kTile * kTile;       // 4096
+constexpr int kTileThreads = 256;
+constexpr int kMergeThreads = 128;
+
+// per-tile record of the bonds that leave the tile (written by k_tile_bonds_label, read by k_tile_merge)
+struct __align__(16) TileBorder {
+    unsigned long long right_col;   // bit y: bond (X0+63, Y0+y) -> (X0+64, Y0+y)
+    unsigned long long bottom_row;  // bit x: bond (X0+x, Y0+63) -> (X0+x, Y0+64)
+};
+
+// ---- shared-memory union-find (tile-local) -----------------------------------------------------
+
+__device__ __forceinline__ uint32_t find_s(volatile uint32_t *parent, uint32_t a)
+{
+    uint32_t p = parent[a];
+    while (p != a) { a = p; p = parent[a]; }
+    return a;
+}
+
+__device__ __forceinline__ void unite_s(volatile uint32_t *parent, uint32_t a, uint32_t b)
+{
+    while (true) {
+        a = find_s(parent, a);
+        b = find_s(parent, b);
+        if (a == b) return;
+        if (a < b) { const uint32_t s = a; a = b; b = s; }
+        const uint32_t old = atomicMin(const_cast<uint32_t *>(parent) + a, b);
+        if (old == a) return;
+        a = old;
+    }
+}
+
+// the four 0x00/0xFF bytes of a __vcmpeq4 result -> 4 bits
+__device__ __forceinline__ uint32_t pack4(uint32_t eq) { return ((eq & 0x01010101u) * 0x01020408u) >> 24; }
+
+// position of the run start (highest set bit of S at or below x)
+__device__ __forceinline__ uint32_t run_start(uint32_t S, uint32_t x) { return 31u - __clz(S & ((2u << x) - 1u)); }
+
+// ---- kernel 1: bonds + tile-local labels --------------------------------------------------------
+
+__global__ void __launch_bounds__(kTileThreads)
+k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
+                   uint32_t *__restrict__ labels, TileBorder *__restrict__ border, Params P)
+{
+    __shared__ uint32_t s_parent[kTileSites];
+    __shared__ uint16_t s_r16[kTile][4];
+    __shared__ uint16_t s_bottom[4];
+    __shared__ uint32_t s_right[2];
+
+    const uint32_t tid = threadIdx.x, y = tid >> 2, c = tid & 3;
+    const uint32_t L = P.L, tiles_x = L >> 6;
+    const uint32_t ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
+    const uint32_t X0 = tx << 6, Y0 = ty << 6;
+    const uint32_t gy = Y0 + y, gx = X0 + (c << 4);
+    const uint64_t row_off = (uint64_t)gy * L;
+    const uint32_t i0 = (uint32_t)(row_off + gx);           // global index of my first site
+
+    if (tid < 2) s_right[tid] = 0;
+
+    // -- spins: my 16 sites, the 16 below them, and the right neighbour of my last site
+    const uint4 sv = *reinterpret_cast<const uint4 *>(spins + row_off + gx);
+    const uint32_t gyd = (gy + 1 == L) ? 0u : gy + 1;
+    const uint4 dv = *reinterpret_cast<const uint4 *>(spins + (uint64_t)gyd * L + gx);
+    uint32_t nxt = __shfl_down_sync(0xFFFFFFFFu, sv.x, 1);
+    if (c == 3) nxt = spins[row_off + ((X0 + kTile == L) ? 0u : X0 + kTile)];
+
+    const uint32_t w[4] = {sv.x, sv.y, sv.z, sv.w};
+    const uint32_t dw[4] = {dv.x, dv.y, dv.z, dv.w};
+    uint32_t eq_r = 0, eq_d = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const uint32_t r = __funnelshift_r(w[k], (k < 3) ? w[k + 1] : nxt, 8);
+        eq_r |= pack4(__vcmpeq4(w[k], r)) << (4 * k);
+        eq_d |= pack4(__vcmpeq4(w[k], dw[k])) << (4 * k);
+    }
+
+    // -- draws: one Philox call per site pair (sites i0+2p, i0+2p+1): words = right, down, right, down
+    uint32_t m_r = 0, m_d = 0;
+    const uint32_t pair0 = i0 >> 1;
+#pragma unroll
+    for (int p = 0; p < 8; ++p) {
+        const uint4 d = philox4x32_10(pair0 + p, 0u, P.t, kPurposeBond, P);
+        m_r |= (uint32_t)(d.x <= P.thr_m1) << (2 * p);
+        m_d |= (uint32_t)(d.y <= P.thr_m1) << (2 * p);
+        m_r |= (uint32_t)(d.z <= P.thr_m1) << (2 * p + 1);
+        m_d |= (uint32_t)(d.w <= P.thr_m1) << (2 * p + 1);
+    }
+    const uint32_t r16 = eq_r & m_r & P.thr_any;
+    const uint32_t d16 = eq_d & m_d & P.thr_any;
+    bonds[i0 >> 4] = r16 | (d16 << 16);
+
+    // -- tile-local masks: bonds that leave the tile are recorded in the border record instead
+    const uint32_t lr16 = (c == 3) ? (r16 & 0x7FFFu) : r16;
+    const uint32_t ld16 = (y == kTile - 1) ? 0u : d16;
+    s_r16[y][c] = (uint16_t)lr16;
+    if (y == kTile - 1) s_bottom[c] = (uint16_t)d16;
+    const uint32_t base = (y << 6) + (c << 4);               // local id of my first site
+    {
+        uint4 *pp = reinterpret_cast<uint4 *>(s_parent + base);
+        pp[0] = make_uint4(base + 0, base + 1, base + 2, base + 3);
+        pp[1] = make_uint4(base + 4, base + 5, base + 6, base + 7);
+        pp[2] = make_uint4(base + 8, base + 9, base + 10, base + 11);
+        pp[3] = make_uint4(base + 12, base + 13, base + 14, base + 15);
+    }
+    __syncthreads();
+    if (c == 3 && (r16 >> 15)) atomicOr(&s_right[y >> 5], 1u << (y & 31));
+
+    // -- unions.  Within my 16 sites a horizontal run is named by its first site (bit tricks);
+    //    only links between runs go through the shared-memory union-find.
+    const uint32_t S = (~(lr16 << 1) | 1u) & 0xFFFFu;        // bit x: site x starts a run in my segment
+    if (c < 3 && (r16 >> 15)) unite_s(s_parent, base + run_start(S, 15), base + 16);
+    if (ld16) {
+        const uint32_t rn = s_r16[y + 1][c];
+        const uint32_t Sn = (~(rn << 1) | 1u) & 0xFFFFu;
+        // bit x is redundant if bit x-1 already joins the same two runs
+        uint32_t v = ld16 & ~(ld16 << 1 & lr16 << 1 & rn << 1);
+        while (v) {
+            const uint32_t x = __ffs(v) - 1;
+            v &= v - 1;
+            unite_s(s_parent, base + run_start(S, x), base + kTile + run_start(Sn, x));
+        }
+    }
+    __syncthreads();
+
+    if (tid == 0) {
+        TileBorder b;
+        b.right_col = (unsigned long long)s_right[0] | ((unsigned long long)s_right[1] << 32);
+        b.bottom_row = (unsigned long long)s_bottom[0] | ((unsigned long long)s_bottom[1] << 16) |
+                       ((unsigned long long)s_bottom[2] << 32) | ((unsigned long long)s_bottom[3] << 48);
+        border[blockIdx.x] = b;
+    }
+
+    // -- labels: global index of the smallest site of my tile-local component
+    const uint32_t origin = Y0 * L + X0;
+    uint32_t lab[16];
+    uint32_t cur = 0;
+#pragma unroll
+    for (int x = 0; x < 16; ++x) {
+        if ((S >> x) & 1u) {
+            const uint32_t r = find_s(s_parent, base + x);
+            cur = origin + (r >> 6) * L + (r & 63u);
+        }
+        lab[x] = cur;
+    }
+    uint4 *lp = reinterpret_cast<uint4 *>(labels + row_off + gx);
+    lp[0] = make_uint4(lab[0], lab[1], lab[2], lab[3]);
+    lp[1] = make_uint4(lab[4], lab[5], lab[6], lab[7]);
+    lp[2] = make_uint4(lab[8], lab[9], lab[10], lab[11]);
+    lp[3] = make_uint4(lab[12], lab[13], lab[14], lab[15]);
+}
+
+// ---- kernel 2: merge across tile borders -------------------------------------------------------
+// One CTA per tile, one thread per border site (64 on the right column, 64 on the bottom row).
+
+__global__ void __launch_bounds__(kMergeThreads)
+k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, Params P)
+{
+    const uint32_t b = threadIdx.x;
+    const uint32_t L = P.L, tiles_x = L >> 6;
+    const uint32_t ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
+    const uint32_t X0 = tx << 6, Y0 = ty << 6;
+    const TileBorder rec = border[blockIdx.x];
+    uint32_t u, v;
+    unsigned long long mask;
+    uint32_t k;
+    if (b < kTile) {
+        k = b; mask = rec.right_col;
+        u = (Y0 + k) * L + X0 + (kTile - 1);
+        v = (Y0 + k) * L + ((X0 + kTile == L) ? 0u : X0 + kTile);
+    } else {
+        k = b - kTile; mask = rec.bottom_row;
+        u = (Y0 + kTile - 1) * L + X0 + k;
+        v = ((Y0 + kTile == L) ? 0u : Y0 + kTile) * L + X0 + k;
+    }
+    const bool on = (mask >> k) & 1ull;
+    uint32_t lu = 0, lv = 0;
+    if (on) { lu = ld_label(labels, u); lv = ld_label(labels, v); }
+    // the previous border bond joins the same two tile-local components: nothing new to learn
+    const uint32_t plu = __shfl_up_sync(0xFFFFFFFFu, lu, 1), plv = __shfl_up_sync(0xFFFFFFFFu, lv, 1);
+    const bool pon = __shfl_up_sync(0xFFFFFFFFu, (uint32_t)on, 1) != 0;
+    const bool dup = (b & 31u) != 0 && pon && plu == lu && plv == lv;
+    if (on && !dup) unite(labels, lu, lv);
+}
+
+// ---- kernel 3: flatten to the canonical root + flip --------------------------------------------
+
+__global__ void __launch_bounds__(kTileThreads)
+k_tile_flip(uint32_t *labels, uint8_t *__restrict__ spins, Params P, int write_labels)
+{
+    __shared__ uint32_t s_lab[kTileSites];
+    __shared__ __align__(16) uint8_t s_state[kTileSites];     // 0xFF = not resolved yet
+    __shared__ uint16_t s_list[kTileSites];
+    __shared__ uint32_t s_count;
+
+    const uint32_t tid = threadIdx.x, y = tid >> 2, c = tid & 3;
+    const uint32_t L = P.L, tiles_x = L >> 6;
+    const uint32_t ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
+    const uint32_t X0 = tx << 6, Y0 = ty << 6;
+    const uint64_t row_off = (uint64_t)(Y0 + y) * L;
+    const uint32_t gx = X0 + (c << 4);
+    const uint32_t i0 = (uint32_t)(row_off + gx);
+    const uint32_t origin = Y0 * L + X0;
+    const uint32_t base = (y << 6) + (c << 4);
+    const uint32_t span = L << 6;                            // 64 rows of the lattice
+
+    if (tid == 0) s_count = 0;
+
+    // -- phase A: stage the tile's labels; find the sites that are roots of the forest (l == i) or
+    //    tile-local roots that the merge hooked under a root outside the tile
+    uint32_t lab[16];
+    {
+        const uint4 *lp = reinterpret_cast<const uint4 *>(labels + row_off + gx);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const uint4 l = lp[k];
+            lab[4 * k] = l.x; lab[4 * k + 1] = l.y; lab[4 * k + 2] = l.z; lab[4 * k + 3] = l.w;
+            reinterpret_cast<uint4 *>(s_lab + base)[k] = l;
+        }
+        *reinterpret_cast<uint4 *>(s_state + base) = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
+    }
+    uint32_t work = 0;
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        const uint32_t l = lab[j];
+        const uint32_t d = l - origin;
+        bool inside = l >= origin && d < span;
+        if (inside) inside = (d - div_L(d, P) * L) < kTile;
+        if (l == i0 + j || !inside) work |= 1u << j;
+    }
+    __syncthreads();
+    if (work) {
+        uint32_t pos = atomicAdd(&s_count, (uint32_t)__popc(work));
+        uint32_t m = work;
+        while (m) {
+            const uint32_t j = __ffs(m) - 1;
+            m &= m - 1;
+            s_list[pos++] = (uint16_t)(base + j);
+        }
+    }
+    __syncthreads();
+
+    // -- phase B: one Philox call per distinct root seen by this tile (work spread over the CTA)
+    const uint32_t count = s_count;
+    for (uint32_t k = tid; k < count; k += kTileThreads) {
+        const uint32_t id = s_list[k];
+        const uint32_t l = s_lab[id];
+        const uint32_t self = origin + (id >> 6) * L + (id & 63u);
+        const uint32_t g = (l == self) ? l : find_root(labels, l);
+        s_lab[id] = g;
+        s_state[id] = (uint8_t)flip_state(g, P);
+    }
+    __syncthreads();
+
+    // -- phase C: every other site reaches a resolved site through in-tile links
+    uint32_t st[4] = {0, 0, 0, 0};
+    uint32_t prev_l = 0, prev_root = 0, prev_s = 0;
+    bool have_prev = false;
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        uint32_t root, s;
+        if ((work >> j) & 1u) {
+            root = s_lab[base + j];
+            s = s_state[base + j];
+        } else if (have_prev && lab[j] == prev_l) {
+            root = prev_root; s = prev_s;
+        } else {
+            uint32_t l = lab[j], id;
+            while (true) {
+                const uint32_t d = l - origin;
+                const uint32_t dy = div_L(d, P);
+                id = (dy << 6) + (d - dy * L);
+                s = s_state[id];
+                l = s_lab[id];
+                if (s != 0xFFu) break;
+            }
+            root = l;
+            prev_l = lab[j]; prev_root = root; prev_s = s; have_prev = true;
+        }
+        lab[j] = root;
+        st[j >> 2] |= s << (8 * (j & 3));
+    }
+    *reinterpret_cast<uint4 *>(spins + row_off + gx) = make_uint4(st[0], st[1], st[2], st[3]);
+    if (write_labels) {
+        uint4 *lp = reinterpret_cast<uint4 *>(labels + row_off + gx);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) lp[k] = make_uint4(lab[4 * k], lab[4 * k + 1], lab[4 * k + 2], lab[4 * k + 3]);
+    }
+}
+
+}  // namespace sw

@@ -160,3 +160,34 @@ def test_state_machine_and_arguments():
     again.set_state(snap, t)
     again.sweep(3)
     assert np.array_equal(again.get_spins(), end)
+
+
+def k_for_threshold(target):
+    """A coupling K whose integer threshold is exactly `target` (bisection on the pinned, monotone map)."""
+    lo, hi = 0.0, 40.0
+    for _ in range(200):
+        mid = 0.5 * (lo + hi)
+        if orc.threshold(mid) < target:
+            lo = mid
+        else:
+            hi = mid
+    assert orc.threshold(hi) == target
+    return hi
+
+
+def test_comparison_is_strict_draw_below_threshold(golden):
+    # north_star: "active iff a uint32 draw is BELOW floor(p*2^32)".  Choose K so that T equals a known
+    # draw exactly: that bond must be inactive, and active once T is one larger.
+    draw = orc.draw_bond(1, 0, 0, 0)
+    assert draw == 0x127BEE41                                  # SURVEY.md sec. 8(c-3) contract example
+    for T, want in ((draw, 0), (draw + 1, 1)):
+        sim = Oracle(4, 2, k_for_threshold(T), 1)
+        sim.init("ordered")
+        sim.sweep(1)
+        assert sim.get_bonds()[0] & 1 == want
+    draw_d = orc.draw_bond(1, 0, 1, 1)                         # down bond of site 1
+    for T, want in ((draw_d, 0), (draw_d + 1, 2)):
+        sim = Oracle(4, 2, k_for_threshold(T), 1)
+        sim.init("ordered")
+        sim.sweep(1)
+        assert sim.get_bonds()[1] & 2 == want

@@ -1,0 +1,218 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle -- needs a B200, `-m gpu`.
+
+Everything compared here is integer work, so the bar is BIT-EXACT: bonds, canonical labels, spins
+and all observables, after every sweep, on the same seeded inputs.  Sizes span several 64x64 tiles,
+non-power-of-two tile counts, the any-L generic path (odd, tiny, L = 2), and the degenerate cases
+(K = 0, K = +inf, q = 255, one cluster, all singletons, adversarial cluster shapes).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle.binding import Oracle
+from paper_1208_2080_b200 import binding as sw
+from paper_1208_2080_b200 import workloads as wl
+from paper_1208_2080_b200.binding import SwendsenWang
+
+pytestmark = pytest.mark.gpu
+
+
+def compare_after_sweep(gpu, cpu, what=""):
+    assert np.array_equal(gpu.get_bonds(), cpu.get_bonds()), f"bonds differ {what}"
+    gl, cl = gpu.get_labels(), cpu.get_labels()
+    if not np.array_equal(gl, cl):
+        bad = np.flatnonzero(gl != cl)
+        raise AssertionError(f"labels differ {what}: {bad.size} sites, first {bad[:8]}, gpu {gl[bad[:8]]}, cpu {cl[bad[:8]]}")
+    assert np.array_equal(gpu.get_spins(), cpu.get_spins()), f"spins differ {what}"
+    assert gpu.measure() == cpu.measure(), f"observables differ {what}"
+
+
+def run_pair(L, q, K, seed, start, sweeps, flags=0, spins=None, t0=0):
+    gpu = SwendsenWang(L, q, K, seed, flags=flags)
+    cpu = Oracle(L, q, K, seed)
+    assert gpu.get_threshold() == cpu.get_threshold()
+    if spins is not None:
+        gpu.set_state(spins, t0); cpu.set_state(spins, t0)
+    else:
+        gpu.init(start); cpu.init(start)
+    assert np.array_equal(gpu.get_spins(), cpu.get_spins()), "initial spins differ"
+    m0 = gpu.measure()
+    assert m0 == cpu.measure() and m0["n_clusters"] == 0
+    for k in range(sweeps):
+        gpu.sweep(1); cpu.sweep(1)
+        assert gpu.get_time() == cpu.get_time()
+        compare_after_sweep(gpu, cpu, f"(L={L} q={q} K={K:.4f} flags={flags} sweep {k})")
+    gpu.close(); cpu.close()
+
+
+# ---------------------------------------------------------------- generic path: any L
+
+@pytest.mark.parametrize("L", [2, 3, 4, 5, 7, 16, 33, 100])
+@pytest.mark.parametrize("q,K", [(2, wl.k_critical(2)), (3, 0.5), (10, wl.k_critical(10))])
+def test_generic_path_small_and_odd_sizes(L, q, K):
+    run_pair(L, q, K, seed=1, start="random", sweeps=4)
+
+
+def test_generic_path_stats():
+    g = SwendsenWang(33, 2, 0.5, 1)
+    st = g.stats()
+    assert st["path"] == 0 and st["kernels_per_sweep"] == 5
+
+
+# ---------------------------------------------------------------- tiled path: L % 64 == 0
+
+@pytest.mark.parametrize("L", [64, 128, 192, 256, 320])
+@pytest.mark.parametrize("q", [2, 3, 4, 10])
+def test_tiled_path_at_criticality(L, q):
+    run_pair(L, q, wl.k_critical(q), seed=1, start="random", sweeps=4)
+
+
+@pytest.mark.parametrize("L", [64, 192, 256])
+@pytest.mark.parametrize("K", [0.0, 0.2, math.log(2.0), 1.5, 4.0, math.inf])
+def test_tiled_path_other_temperatures_from_an_ordered_start(L, K):
+    run_pair(L, 2, K, seed=3, start="ordered", sweeps=3)
+
+
+@pytest.mark.parametrize("flags", [sw.FLAG_LAZY_LABELS, sw.FLAG_FORCE_GENERIC, sw.FLAG_FORCE_GENERIC | sw.FLAG_LAZY_LABELS])
+def test_flag_variants_give_identical_results(flags):
+    run_pair(128, 3, wl.k_critical(3), seed=5, start="random", sweeps=3, flags=flags)
+    run_pair(192, 2, wl.k_critical(2), seed=5, start="ordered", sweeps=3, flags=flags)
+
+
+def test_tiled_path_is_selected_and_counts_kernels():
+    g = SwendsenWang(128, 2, 0.5, 1)
+    g.init("ordered")
+    g.sweep(3)
+    g.synchronize()
+    st = g.stats()
+    assert st["path"] == 1 and (st["tile_w"], st["tile_h"]) == (64, 64) and st["kernels_per_sweep"] == 3
+    assert st["kernel_launches"] == 9 and st["sweeps"] == 3
+
+
+def test_q255_and_large_seed():
+    run_pair(64, 255, 2.0, seed=0xFEDCBA9876543210, start="random", sweeps=3)
+    run_pair(9, 255, 2.0, seed=0xFEDCBA9876543210, start="random", sweeps=3)
+
+
+def test_late_sweep_counter():
+    rng_spins = wl.spins_uniform_random(128, 3, 11)
+    run_pair(128, 3, 1.0, seed=2, start=None, sweeps=2, spins=rng_spins, t0=0xFFFFFFF0)
+
+
+# ---------------------------------------------------------------- adversarial cluster shapes
+
+@pytest.mark.parametrize("L", [64, 192, 256])
+@pytest.mark.parametrize("K", [math.inf, 2.0])
+def test_adversarial_lattices_tiled(L, K):
+    for name, spins in wl.crafted_lattices(L, 3).items():
+        gpu = SwendsenWang(L, 3, K, 1)
+        cpu = Oracle(L, 3, K, 1)
+        gpu.set_state(spins, 5); cpu.set_state(spins, 5)
+        gpu.sweep(1); cpu.sweep(1)
+        compare_after_sweep(gpu, cpu, f"({name}, L={L}, K={K})")
+        gpu.close(); cpu.close()
+
+
+@pytest.mark.parametrize("L", [6, 31, 96])
+def test_adversarial_lattices_generic(L):
+    flags = sw.FLAG_FORCE_GENERIC
+    for name, spins in wl.crafted_lattices(L, 3).items():
+        gpu = SwendsenWang(L, 3, math.inf, 1, flags=flags)
+        cpu = Oracle(L, 3, math.inf, 1)
+        gpu.set_state(spins, 0); cpu.set_state(spins, 0)
+        gpu.sweep(1); cpu.sweep(1)
+        compare_after_sweep(gpu, cpu, f"({name}, L={L})")
+
+
+def test_long_snake_through_every_tile():
+    # the spiral path at L = 512 crosses tile borders ~ 4000 times and has diameter ~ 130 000
+    L = 512
+    spins = wl.spins_spiral(L)
+    gpu = SwendsenWang(L, 2, math.inf, 1)
+    cpu = Oracle(L, 2, math.inf, 1)
+    gpu.set_state(spins, 0); cpu.set_state(spins, 0)
+    gpu.sweep(1); cpu.sweep(1)
+    compare_after_sweep(gpu, cpu, "(spiral 512)")
+
+
+# ---------------------------------------------------------------- BASELINE.json configs
+
+def test_config1_L256_q2_every_sweep():
+    c = wl.CONFIGS["c1_L256_q2"]
+    gpu = SwendsenWang(c["L"], c["q"], c["K"], c["seed"])
+    cpu = Oracle(c["L"], c["q"], c["K"], c["seed"])
+    gpu.init(c["start"]); cpu.init(c["start"])
+    for k in range(c["sweeps"]):
+        gpu.sweep(1); cpu.sweep(1)
+        if k < 5 or k % 20 == 19:
+            compare_after_sweep(gpu, cpu, f"(config 1 sweep {k})")
+        else:
+            assert np.array_equal(gpu.get_spins(), cpu.get_spins()), f"config 1 sweep {k}"
+            assert gpu.measure() == cpu.measure(), f"config 1 sweep {k}"
+
+
+def test_config1_series_call_matches_oracle_series():
+    c = wl.CONFIGS["c1_L256_q2"]
+    gpu = SwendsenWang(c["L"], c["q"], c["K"], c["seed"])
+    cpu = Oracle(c["L"], c["q"], c["K"], c["seed"])
+    gpu.init(c["start"]); cpu.init(c["start"])
+    assert np.array_equal(gpu.sweep_measure(c["sweeps"]), cpu.sweep_measure(c["sweeps"]))
+    assert np.array_equal(gpu.get_spins(), cpu.get_spins())
+
+
+@pytest.mark.parametrize("name,sweeps", [("c2_L4096_q2", 3)])
+def test_config2_L4096_first_sweeps(name, sweeps):
+    c = wl.CONFIGS[name]
+    sweeps = int(os.environ.get("SW_C2_SWEEPS", sweeps))
+    run_pair(c["L"], c["q"], c["K"], c["seed"], c["start"], sweeps)
+
+
+@pytest.mark.parametrize("q", [3, 4, 10])
+def test_configs_3_4_shapes_at_reduced_L(q):
+    # configs 3 and 4 (q = 3, 4 at L = 8192; q = 10 at L = 16384 above/below K_c) at L = 1024, where the
+    # oracle finishes in seconds; the full sizes are covered by test_full_size_gpu.py
+    for K in ([wl.k_critical(q)] if q < 10 else [wl.k_critical(10) * 1.005, wl.k_critical(10) * 0.995]):
+        run_pair(1024, q, K, seed=1, start="random", sweeps=2)
+
+
+# ---------------------------------------------------------------- state machine / errors through the ABI
+
+def test_state_machine_and_errors():
+    g = SwendsenWang(64, 2, 0.5, 1)
+    with pytest.raises(sw.SwError) as e:
+        g.sweep(1)
+    assert e.value.code == sw.ERR_STATE
+    g.init("random")
+    with pytest.raises(sw.SwError) as e:
+        g.get_labels()
+    assert e.value.code == sw.ERR_STATE
+    with pytest.raises(sw.SwError) as e:
+        g.set_state(np.full(64 * 64, 2, dtype=np.uint8), 0)
+    assert e.value.code == sw.ERR_INVALID_ARG
+    with pytest.raises(sw.SwError):
+        g.sweep(1)                                   # the rejected state left no spins
+    g.init("ordered")
+    g.sweep(2)
+    snap, t = g.get_spins().copy(), g.get_time()
+    g.sweep(3)
+    end = g.get_spins().copy()
+    h = SwendsenWang(64, 2, 0.5, 1, use_torch=False)    # library-owned memory and stream
+    h.set_state(snap, t)
+    h.sweep(3)
+    assert np.array_equal(h.get_spins(), end)
+    assert np.array_equal(h.get_rows("labels", 10, 7), g.get_labels().reshape(64, 64)[10:17])
+    assert np.array_equal(h.get_rows("bonds", 60, 4), g.get_bonds().reshape(64, 64)[60:64])
+    assert np.array_equal(h.get_rows("spins", 0, 64).reshape(-1), end)
+
+
+def test_profile_slots():
+    g = SwendsenWang(256, 2, wl.k_critical(2), 1)
+    g.init("random")
+    g.sweep(2)
+    g.profile_begin()
+    g.sweep(5)
+    prof = g.profile_end()
+    assert set(prof) == {"k_tile_bonds_label", "k_tile_merge", "k_tile_flip"}
+    assert all(v["launches"] == 5 and v["ms"] > 0 for v in prof.values())
