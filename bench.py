@@ -1,0 +1,352 @@
+#!/usr/bin/env python
+"""bench.py -- spin flips per nanosecond of the Swendsen-Wang sweep on B200 (one JSON line).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl reference]
+
+A step is ONE full sweep (bond activation, tile-local labeling, border merge, flatten to canonical
+labels, flip: SURVEY.md sec. 8(a) rows a1-a5) of the headline workload of BASELINE.json: q = 2 Potts at
+K_c on the 65536 x 65536 periodic lattice (2^32 sites), random start, Philox seed 1.  W untimed sweeps,
+then exactly K sweeps timed with CUDA events on the stream the kernels run on.  The 21 GiB working
+set is far larger than the 126 MB L2, so no L2 flush is needed between sweeps.
+
+N > 1: the path does not shard without collectives ("replicas only"), so every
+rank runs an independent replica (seed 1 + rank) and the value is the aggregate of all replicas
+over the slowest rank's time.
+
+--impl reference times the CPU oracle (oracle/, plain single-threaded C++) on the host cores on a
+bounded sample of the same workload; it is a deliberately slow reference program, not a target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1208_2080_b200 import workloads as wl  # noqa: E402
+
+METRIC = "spin_flips_per_ns"
+UNIT = "flips/ns"
+PAPER_FLIPS_PER_NS = 37.30        # PAPER.md:103 (Table 1): L = 65536, q = 2, T_c, 256 x Tesla M2050
+HBM_FALLBACK_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+
+# Algorithmic bytes per site per launch.
+BYTES_PER_SITE = {
+    "k_tile_bonds_label": 1.0 + 0.25 + 4.0 + 16.0 / 4096.0,   # spins R, bond bits W, labels W, border record W
+    "k_tile_merge": 16.0 / 4096.0 + 2 * 4.0 * 2.0 / 64.0 * 0.5,  # border record R + two label reads per ACTIVE border bond (~half)
+    "k_tile_flip": 4.0 + 4.0 + 1.0,                           # labels R, canonical labels W, spins W
+}
+BYTES_PER_SITE_LAZY = dict(BYTES_PER_SITE, k_tile_flip=4.0 + 1.0)
+
+
+def rank_info():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons while the timed region runs."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc, self.thread = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "100", "-i", str(self.index)],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for (ts, r) in self.rows if t0 - 0.05 <= ts <= t1 + 0.15] or [r for (_, r) in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def hbm_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy bandwidth)"
+    except Exception:
+        return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(workload, kernel):
+    """DRAM bytes per launch of `kernel` from the committed ncu summary, if one exists for this workload."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            return json.load(f).get(workload, {}).get(kernel)
+    except Exception:
+        return None
+
+
+def time_oracle(L, q, K, seed, start, warm, sweeps):
+    from oracle.binding import Oracle
+    sim = Oracle(L, q, K, seed)
+    sim.init(start)
+    if warm:
+        sim.sweep(warm)
+    t0 = time.perf_counter()
+    sim.sweep(sweeps)
+    dt = time.perf_counter() - t0
+    sim.close()
+    return dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, one thread, on a bounded sample of the workload."""
+    rank, _, world = rank_info()
+    if rank != 0:
+        return 0
+    c = wl.CONFIGS[args.workload]
+    L = min(c["L"], args.reference_L)
+    from oracle.binding import Oracle
+    sim = Oracle(L, c["q"], c["K"], c["seed"])
+    sim.init(c["start"])
+    sim.sweep(args.warmup)
+    t0 = time.perf_counter()
+    sim.sweep(args.steps)
+    dt = time.perf_counter() - t0
+    value = L * L * args.steps / dt / 1e9
+    sample = (f"oracle/libsw_oracle.so, 1 thread, each step = one sweep of an L={L} lattice with the workload's q, K, "
+              f"start and seed ({L * L} of the workload's {c['L'] ** 2} sites)")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": args.workload, "L": c["L"], "q": c["q"], "K": c["K"], "start": c["start"], "seed": c["seed"],
+                   "sample_L": L},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+    return 0
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_1208_2080_b200.binding import FLAG_DEFAULT, FLAG_LAZY_LABELS, SwendsenWang
+
+    rank, local_rank, world = rank_info()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU path (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    distributed = world > 1
+    if distributed:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    c = dict(wl.CONFIGS[args.workload])
+    L, q, K = c["L"], c["q"], c["K"]
+    N = L * L
+    flags = FLAG_LAZY_LABELS if args.lazy else FLAG_DEFAULT
+    sim = SwendsenWang(L, q, K, c["seed"] + rank, flags=flags)
+    sim.init(c["start"])
+    sim.sweep(args.warmup)
+    sim.synchronize()
+
+    def barrier():
+        if distributed:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- timed region: exactly K sweeps, CUDA events on the stream the kernels are enqueued on
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    launches0 = sim.stats()["kernel_launches"]
+    per_kernel_in_region = N >= (1 << 24)          # event overhead (~us per kernel) is negligible only for big lattices
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    wall0 = time.time()
+    if per_kernel_in_region:
+        sim.profile_begin()
+    ev0.record()
+    sim.sweep(args.steps)
+    ev1.record()
+    prof = sim.profile_end() if per_kernel_in_region else None
+    barrier()
+    wall1 = time.time()
+    elapsed_ms = ev0.elapsed_time(ev1)
+    launches = sim.stats()["kernel_launches"] - launches0
+    clocks = sampler.stop(wall0, wall1) if rank == 0 else None
+    if distributed:
+        tmax = torch.tensor([elapsed_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        elapsed_ms = float(tmax.item())
+    value = world * N * args.steps / (elapsed_ms * 1e-3) / 1e9
+
+    if not per_kernel_in_region:                   # small lattice: separate pass for the per-kernel split
+        sim.profile_begin()
+        sim.sweep(args.steps)
+        prof = sim.profile_end()
+
+    # ---- update + measurement (the paper's second column): sweep + all observables each step
+    m_steps = max(1, min(args.steps, 10))
+    sim.measure(largest=False)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(m_steps):
+        sim.sweep(1)
+        obs = sim.measure(largest=False)
+    e1.record()
+    torch.cuda.synchronize()
+    value_meas = N * m_steps / (e0.elapsed_time(e1) * 1e-3) / 1e9
+
+    # ---- end to end through the C ABI with HOST buffers: H2D of the spins, one sweep, D2H of the new spins
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    host = torch.empty(N, dtype=torch.uint8, pin_memory=True)
+    sim.get_spins_ptr(host.data_ptr())
+    t_now = sim.get_time()
+    barrier()
+    w0 = time.perf_counter()
+    for k in range(e2e_steps):
+        sim.set_state_ptr(host.data_ptr(), t_now + k)      # H2D (+ on-device validation of the spin values)
+        sim.sweep(1)
+        sim.get_spins_ptr(host.data_ptr())                 # D2H; synchronises
+    barrier()
+    e2e_s = time.perf_counter() - w0
+    if distributed:
+        tmax = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        e2e_s = float(tmax.item())
+    e2e_value = world * N * e2e_steps / e2e_s / 1e9
+
+    stats = sim.stats()
+    if rank != 0:
+        if distributed:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel
+    peak, peak_src = hbm_peak()
+    bps = BYTES_PER_SITE_LAZY if args.lazy else BYTES_PER_SITE
+    kernels = {}
+    for name, rec in (prof or {}).items():
+        avg_ms = rec["ms"] / rec["launches"]
+        b = bps.get(name)
+        kernels[name] = {"ms_per_launch": avg_ms, "share": None,
+                         "algorithmic_bytes_per_site": b,
+                         "achieved_gbs": (b * N / (avg_ms * 1e-3) / 1e9) if b else None}
+    tot = sum(k["ms_per_launch"] for k in kernels.values()) or 1.0
+    for k in kernels.values():
+        k["share"] = k["ms_per_launch"] / tot
+    roofline = None
+    if kernels:
+        top = max(kernels, key=lambda n: kernels[n]["ms_per_launch"])
+        a = kernels[top]["achieved_gbs"]
+        roofline = {"kernel": top, "bound": "hbm", "achieved": a, "peak": peak, "unit": "GB/s",
+                    "frac": (a / peak) if a else None, "traffic": ncu_traffic(args.workload, top),
+                    "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": bps.get(top, 0) * N}
+    sweep_bytes = sum(v for v in bps.values()) * N
+    sweep_floor_ms = sweep_bytes / (peak * 1e9) * 1e3
+    per_gpu_ms = elapsed_ms / args.steps
+
+    # ---- the oracle on this box's host cores (reported baseline, rank 0, N = 1 only)
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu_baseline:
+        Lc = min(L, args.cpu_baseline_L)
+        dt = time_oracle(Lc, q, K, c["seed"], c["start"], 1, args.cpu_baseline_sweeps)
+        cpu_baseline = {"value": Lc * Lc * args.cpu_baseline_sweeps / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+                        "host_cores_available": os.cpu_count(),
+                        "sample": f"{args.cpu_baseline_sweeps} sweeps of an L={Lc} lattice (q={q}, K=K_c, {c['start']} start, seed {c['seed']}) "
+                                  f"after 1 warm-up sweep, single thread, {dt:.1f} s"}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": per_gpu_ms, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": (value / PAPER_FLIPS_PER_NS) if args.workload == wl.HEADLINE else None,
+        "dtype": "u32", "data": "synthetic",
+        "config": {"workload": args.workload, "L": L, "q": q, "K": K, "start": c["start"], "seed": c["seed"],
+                   "labels": "lazy" if args.lazy else "canonical every sweep",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "l2": f"working set {stats['device_bytes'] / 2**30:.1f} GiB >> 126 MB L2, no flush needed" if stats["device_bytes"] > (1 << 30)
+                         else "working set fits L2: HBM roofline fractions are not meaningful at this size"},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N, "d2h_bytes_per_step": N, "steps": e2e_steps,
+                "what": "sw_set_state(host spins) + sw_sweep(1) + sw_get_spins(host) per step, pinned host memory"},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "cpu_baseline": cpu_baseline,
+        "kernels": kernels,
+        "sweep_model": {"bytes_per_site": sum(bps.values()), "floor_ms_at_peak": sweep_floor_ms,
+                        "frac_of_min_traffic_roofline": sweep_floor_ms / per_gpu_ms},
+        "update_plus_measurement": {"value": value_meas, "unit": UNIT, "steps": m_steps,
+                                    "what": "sw_sweep(1) + sw_measure(energy, magnetisation, n_clusters) per step"},
+        "last_observables": obs,
+        "paper_context": {"flips_per_ns_256xM2050_L65536": PAPER_FLIPS_PER_NS, "flips_per_ns_1xM2050_L4096": 0.232,
+                          "source": "PAPER.md:97-103 (Table 1)"},
+    }
+    print(json.dumps(out))
+    if distributed:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--workload", choices=sorted(wl.CONFIGS), default=wl.HEADLINE)
+    ap.add_argument("--lazy", action="store_true", help="SW_FLAG_LAZY_LABELS: canonical labels flattened on demand only")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-baseline-L", type=int, default=4096)
+    ap.add_argument("--cpu-baseline-sweeps", type=int, default=4)
+    ap.add_argument("--reference-L", type=int, default=2048)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = 20 if args.steps is None else args.steps
+        args.warmup = 5 if args.warmup is None else args.warmup
+        return run_reference(args)
+    args.steps = 40 if args.steps is None else args.steps
+    args.warmup = 60 if args.warmup is None else args.warmup
+    return run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

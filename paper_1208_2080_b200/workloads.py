@@ -31,6 +31,9 @@ CONFIGS = {
     "c4_L16384_q10_below": dict(L=16384, q=10, K=k_critical(10) * 0.995, start="random", sweeps=200, seed=1),
     "c5_L65536_q2": dict(L=65536, q=2, K=k_critical(2), start="random", sweeps=100, seed=1),
 }
+# not a BASELINE.json config: the headline physics at a size whose working set (1.3 GiB) is well beyond
+# the L2 but small enough for an `ncu --set full` capture (ncu replays each kernel ~40 times)
+CONFIGS["p_L16384_q2"] = dict(L=16384, q=2, K=k_critical(2), start="random", sweeps=100, seed=1)
 HEADLINE = "c5_L65536_q2"
 
 
