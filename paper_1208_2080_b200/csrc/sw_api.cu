@@ -30,7 +30,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Plan {
-    size_t spins, bonds, labels, border, row, flag, total;   // byte offsets into the workspace
+    size_t spins, bonds, labels, rootbits, border, row, flag, total;   // byte offsets into the workspace
 };
 
 bool tiled_ok(uint32_t L, uint32_t flags) { return (L % sw::kTile == 0) && !(flags & SW_FLAG_FORCE_GENERIC); }
@@ -43,6 +43,7 @@ Plan make_plan(uint32_t L, uint32_t q, uint32_t flags)
     p.spins = off;  off = align_up(off + N);
     p.bonds = off;  off = align_up(off + ((N + 15) / 16) * 4);
     p.labels = off; off = align_up(off + N * 4);
+    p.rootbits = off; off = align_up(off + (tiled_ok(L, flags) ? (N / 16) * 2 : 0));
     p.border = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileBorder) : 0));
     p.row = off;    off = align_up(off + (3 + (size_t)q) * 8);
     p.flag = off;   off = align_up(off + 4);
@@ -65,6 +66,7 @@ struct sw_ctx {
     size_t ws_bytes = 0;
     uint8_t *d_spins = nullptr;
     uint32_t *d_bonds = nullptr, *d_labels = nullptr, *d_flag = nullptr;
+    uint16_t *d_rootbits = nullptr;
     sw::TileBorder *d_border = nullptr;
     unsigned long long *d_row = nullptr;
     uint32_t *d_sizes = nullptr;          // lazily allocated 4N-byte scratch for cluster sizes
@@ -149,11 +151,11 @@ int sweep_once(sw_ctx *c)
     if (c->tiled) {
         const unsigned tiles = (unsigned)(c->N / sw::kTileSites);
         { Timed tm(c, SLOT_TILE);
-          sw::k_tile_bonds_label<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_border, P); }
+          sw::k_tile_bonds_label<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, P); }
         { Timed tm(c, SLOT_MERGE);
           sw::k_tile_merge<<<tiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, P); }
         { Timed tm(c, SLOT_FLIP);
-          sw::k_tile_flip<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_labels, c->d_spins, P, c->lazy ? 0 : 1); }
+          sw::k_tile_flip<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->lazy ? 0 : 1); }
         c->labels_flat = !c->lazy;
     } else {
         const int th = 256;
@@ -250,6 +252,7 @@ int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed,
     c->d_spins = c->ws + plan.spins;
     c->d_bonds = (uint32_t *)(c->ws + plan.bonds);
     c->d_labels = (uint32_t *)(c->ws + plan.labels);
+    c->d_rootbits = (uint16_t *)(c->ws + plan.rootbits);
     c->d_border = (sw::TileBorder *)(c->ws + plan.border);
     c->d_row = (unsigned long long *)(c->ws + plan.row);
     c->d_flag = (uint32_t *)(c->ws + plan.flag);

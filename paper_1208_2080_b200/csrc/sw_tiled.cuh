@@ -27,11 +27,20 @@ struct __align__(16) TileBorder {
 };
 
 // ---- shared-memory union-find (tile-local) -----------------------------------------------------
+// Links always point to a smaller local id, so plain stores that replace a link by a link to an
+// ancestor (path halving) are safe next to concurrent atomicMin hooks: nothing that was joined
+// can come apart, and the root of a set is always its smallest member.
 
 __device__ __forceinline__ uint32_t find_s(volatile uint32_t *parent, uint32_t a)
 {
     uint32_t p = parent[a];
-    while (p != a) { a = p; p = parent[a]; }
+    while (p != a) {
+        const uint32_t gp = parent[p];
+        if (gp == p) return p;
+        parent[a] = gp;                                   // path halving
+        a = gp;
+        p = parent[a];
+    }
     return a;
 }
 
@@ -56,14 +65,19 @@ __device__ __forceinline__ uint32_t run_start(uint32_t S, uint32_t x) { return 3
 
 // ---- kernel 1: bonds + tile-local labels --------------------------------------------------------
 
+constexpr uint32_t kMaxLinks = 63 * 64 + 3 * 64;      // every vertical bond + every segment joint of a tile
+
 __global__ void __launch_bounds__(kTileThreads)
 k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
-                   uint32_t *__restrict__ labels, TileBorder *__restrict__ border, Params P)
+                   uint32_t *__restrict__ labels, uint16_t *__restrict__ rootbits,
+                   TileBorder *__restrict__ border, Params P)
 {
     __shared__ uint32_t s_parent[kTileSites];
+    __shared__ uint32_t s_links[kMaxLinks];
     __shared__ uint16_t s_r16[kTile][4];
     __shared__ uint16_t s_bottom[4];
     __shared__ uint32_t s_right[2];
+    __shared__ uint32_t s_nlinks;
 
     const uint32_t tid = threadIdx.x, y = tid >> 2, c = tid & 3;
     const uint32_t L = P.L, tiles_x = L >> 6;
@@ -74,6 +88,7 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
     const uint32_t i0 = (uint32_t)(row_off + gx);           // global index of my first site
 
     if (tid < 2) s_right[tid] = 0;
+    if (tid == 2) s_nlinks = 0;
 
     // -- spins: my 16 sites, the 16 below them, and the right neighbour of my last site
     const uint4 sv = *reinterpret_cast<const uint4 *>(spins + row_off + gx);
@@ -123,19 +138,35 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
     __syncthreads();
     if (c == 3 && (r16 >> 15)) atomicOr(&s_right[y >> 5], 1u << (y & 31));
 
-    // -- unions.  Within my 16 sites a horizontal run is named by its first site (bit tricks);
-    //    only links between runs go through the shared-memory union-find.
+    // -- links.  Within my 16 sites a horizontal run is named by its first site (bit tricks); only
+    //    links between runs go through the shared-memory union-find.  They are first gathered in a
+    //    CTA-wide list so that the union loop below runs with all lanes busy.
     const uint32_t S = (~(lr16 << 1) | 1u) & 0xFFFFu;        // bit x: site x starts a run in my segment
-    if (c < 3 && (r16 >> 15)) unite_s(s_parent, base + run_start(S, 15), base + 16);
-    if (ld16) {
-        const uint32_t rn = s_r16[y + 1][c];
-        const uint32_t Sn = (~(rn << 1) | 1u) & 0xFFFFu;
-        // bit x is redundant if bit x-1 already joins the same two runs
-        uint32_t v = ld16 & ~(ld16 << 1 & lr16 << 1 & rn << 1);
-        while (v) {
-            const uint32_t x = __ffs(v) - 1;
-            v &= v - 1;
-            unite_s(s_parent, base + run_start(S, x), base + kTile + run_start(Sn, x));
+    {
+        const bool joint = c < 3 && (r16 >> 15);             // my last site is bonded to the next segment
+        uint32_t v = 0, Sn = 0;
+        if (ld16) {
+            const uint32_t rn = s_r16[y + 1][c];
+            Sn = (~(rn << 1) | 1u) & 0xFFFFu;
+            v = ld16 & ~(ld16 << 1 & lr16 << 1 & rn << 1);   // bit x is redundant if bit x-1 joins the same two runs
+        }
+        const uint32_t n = __popc(v) + (joint ? 1u : 0u);
+        if (n) {
+            uint32_t pos = atomicAdd(&s_nlinks, n);
+            if (joint) s_links[pos++] = (base + run_start(S, 15)) | ((base + 16) << 16);
+            while (v) {
+                const uint32_t x = __ffs(v) - 1;
+                v &= v - 1;
+                s_links[pos++] = (base + run_start(S, x)) | ((base + kTile + run_start(Sn, x)) << 16);
+            }
+        }
+    }
+    __syncthreads();
+    {
+        const uint32_t n = s_nlinks;
+        for (uint32_t k = tid; k < n; k += kTileThreads) {
+            const uint32_t e = s_links[k];
+            unite_s(s_parent, e & 0xFFFFu, e >> 16);
         }
     }
     __syncthreads();
@@ -148,15 +179,29 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
         border[blockIdx.x] = b;
     }
 
-    // -- labels: global index of the smallest site of my tile-local component
+    // -- compress: every entry points straight at its root (no hooks happen any more)
+#pragma unroll 4
+    for (uint32_t j = 0; j < 16; ++j) {
+        const uint32_t id = tid + j * kTileThreads;
+        const uint32_t p = s_parent[id];
+        if (p != id) {                                       // read-only chase: other threads finalise entries now
+            uint32_t r = p, g = const_cast<volatile uint32_t *>(s_parent)[r];
+            while (g != r) { r = g; g = const_cast<volatile uint32_t *>(s_parent)[r]; }
+            if (r != p) s_parent[id] = r;
+        }
+    }
+    __syncthreads();
+
+    // -- labels: global index of the smallest site of my tile-local component; root flags
     const uint32_t origin = Y0 * L + X0;
     uint32_t lab[16];
-    uint32_t cur = 0;
+    uint32_t cur = 0, roots = 0;
 #pragma unroll
     for (int x = 0; x < 16; ++x) {
         if ((S >> x) & 1u) {
-            const uint32_t r = find_s(s_parent, base + x);
+            const uint32_t r = s_parent[base + x];
             cur = origin + (r >> 6) * L + (r & 63u);
+            roots |= (r == base + x) ? (1u << x) : 0u;
         }
         lab[x] = cur;
     }
@@ -165,6 +210,7 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
     lp[1] = make_uint4(lab[4], lab[5], lab[6], lab[7]);
     lp[2] = make_uint4(lab[8], lab[9], lab[10], lab[11]);
     lp[3] = make_uint4(lab[12], lab[13], lab[14], lab[15]);
+    rootbits[i0 >> 4] = (uint16_t)roots;
 }
 
 // ---- kernel 2: merge across tile borders -------------------------------------------------------
@@ -201,12 +247,18 @@ k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, Params P)
 }
 
 // ---- kernel 3: flatten to the canonical root + flip --------------------------------------------
+// After the merge, labels[] is a forest: a site that is not the root of its tile-local component
+// points at that root (inside the tile); a tile-local root points at itself or, if the merge hooked
+// it, at a smaller root anywhere.  `rootbits` says which sites are tile-local roots, so each
+// distinct root seen by the tile is chased and drawn ONCE (work spread over the whole CTA) and
+// every other site needs one shared-memory lookup.
 
 __global__ void __launch_bounds__(kTileThreads)
-k_tile_flip(uint32_t *labels, uint8_t *__restrict__ spins, Params P, int write_labels)
+k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__restrict__ spins,
+            Params P, int write_labels)
 {
-    __shared__ uint32_t s_lab[kTileSites];
-    __shared__ __align__(16) uint8_t s_state[kTileSites];     // 0xFF = not resolved yet
+    __shared__ uint32_t s_root[kTileSites];                   // per tile-local root: its canonical root
+    __shared__ uint8_t s_state[kTileSites];                   // per tile-local root: the new state
     __shared__ uint16_t s_list[kTileSites];
     __shared__ uint32_t s_count;
 
@@ -219,12 +271,10 @@ k_tile_flip(uint32_t *labels, uint8_t *__restrict__ spins, Params P, int write_l
     const uint32_t i0 = (uint32_t)(row_off + gx);
     const uint32_t origin = Y0 * L + X0;
     const uint32_t base = (y << 6) + (c << 4);
-    const uint32_t span = L << 6;                            // 64 rows of the lattice
 
     if (tid == 0) s_count = 0;
 
-    // -- phase A: stage the tile's labels; find the sites that are roots of the forest (l == i) or
-    //    tile-local roots that the merge hooked under a root outside the tile
+    // -- phase A: my 16 labels; queue the tile-local roots among them
     uint32_t lab[16];
     {
         const uint4 *lp = reinterpret_cast<const uint4 *>(labels + row_off + gx);
@@ -232,70 +282,43 @@ k_tile_flip(uint32_t *labels, uint8_t *__restrict__ spins, Params P, int write_l
         for (int k = 0; k < 4; ++k) {
             const uint4 l = lp[k];
             lab[4 * k] = l.x; lab[4 * k + 1] = l.y; lab[4 * k + 2] = l.z; lab[4 * k + 3] = l.w;
-            reinterpret_cast<uint4 *>(s_lab + base)[k] = l;
         }
-        *reinterpret_cast<uint4 *>(s_state + base) = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
     }
-    uint32_t work = 0;
-#pragma unroll
-    for (int j = 0; j < 16; ++j) {
-        const uint32_t l = lab[j];
-        const uint32_t d = l - origin;
-        bool inside = l >= origin && d < span;
-        if (inside) inside = (d - div_L(d, P) * L) < kTile;
-        if (l == i0 + j || !inside) work |= 1u << j;
-    }
+    const uint32_t work = rootbits[i0 >> 4];
     __syncthreads();
     if (work) {
         uint32_t pos = atomicAdd(&s_count, (uint32_t)__popc(work));
-        uint32_t m = work;
-        while (m) {
-            const uint32_t j = __ffs(m) - 1;
-            m &= m - 1;
-            s_list[pos++] = (uint16_t)(base + j);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            if ((work >> j) & 1u) {
+                s_root[base + j] = lab[j];
+                s_list[pos++] = (uint16_t)(base + j);
+            }
         }
     }
     __syncthreads();
 
-    // -- phase B: one Philox call per distinct root seen by this tile (work spread over the CTA)
+    // -- phase B: one chase + one Philox call per tile-local root
     const uint32_t count = s_count;
     for (uint32_t k = tid; k < count; k += kTileThreads) {
         const uint32_t id = s_list[k];
-        const uint32_t l = s_lab[id];
+        const uint32_t l = s_root[id];
         const uint32_t self = origin + (id >> 6) * L + (id & 63u);
         const uint32_t g = (l == self) ? l : find_root(labels, l);
-        s_lab[id] = g;
+        s_root[id] = g;
         s_state[id] = (uint8_t)flip_state(g, P);
     }
     __syncthreads();
 
-    // -- phase C: every other site reaches a resolved site through in-tile links
+    // -- phase C: every site looks its tile-local root up
     uint32_t st[4] = {0, 0, 0, 0};
-    uint32_t prev_l = 0, prev_root = 0, prev_s = 0;
-    bool have_prev = false;
 #pragma unroll
     for (int j = 0; j < 16; ++j) {
-        uint32_t root, s;
-        if ((work >> j) & 1u) {
-            root = s_lab[base + j];
-            s = s_state[base + j];
-        } else if (have_prev && lab[j] == prev_l) {
-            root = prev_root; s = prev_s;
-        } else {
-            uint32_t l = lab[j], id;
-            while (true) {
-                const uint32_t d = l - origin;
-                const uint32_t dy = div_L(d, P);
-                id = (dy << 6) + (d - dy * L);
-                s = s_state[id];
-                l = s_lab[id];
-                if (s != 0xFFu) break;
-            }
-            root = l;
-            prev_l = lab[j]; prev_root = root; prev_s = s; have_prev = true;
-        }
-        lab[j] = root;
-        st[j >> 2] |= s << (8 * (j & 3));
+        const uint32_t d = (((work >> j) & 1u) ? i0 + j : lab[j]) - origin;
+        const uint32_t dy = div_L(d, P);
+        const uint32_t id = (dy << 6) + (d - dy * L);
+        lab[j] = s_root[id];
+        st[j >> 2] |= (uint32_t)s_state[id] << (8 * (j & 3));
     }
     *reinterpret_cast<uint4 *>(spins + row_off + gx) = make_uint4(st[0], st[1], st[2], st[3]);
     if (write_labels) {
