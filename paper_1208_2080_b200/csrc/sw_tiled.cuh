@@ -65,7 +65,12 @@ __device__ __forceinline__ uint32_t run_start(uint32_t S, uint32_t x) { return 3
 
 // ---- kernel 1: bonds + tile-local labels --------------------------------------------------------
 
-constexpr uint32_t kMaxLinks = 63 * 64 + 3 * 64;      // every vertical bond + every segment joint of a tile
+// A warp owns the 8 tile rows 8w .. 8w+7 (its "strip").  Links inside a strip are united by that
+// warp alone, in row order (which keeps the trees shallow, as in a sequential Hoshen-Kopelman
+// sweep); the links between strips are united by the whole CTA afterwards.
+constexpr uint32_t kStripLinks = 7 * 64 + 8 * 3;      // vertical bonds inside a strip + its segment joints = 472
+constexpr uint32_t kStripCap = 480;
+constexpr uint32_t kSeamLinks = 7 * 64;               // vertical bonds between strips
 
 __global__ void __launch_bounds__(kTileThreads)
 k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
@@ -73,13 +78,15 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
                    TileBorder *__restrict__ border, Params P)
 {
     __shared__ uint32_t s_parent[kTileSites];
-    __shared__ uint32_t s_links[kMaxLinks];
+    __shared__ uint32_t s_links[kTileThreads / 32][kStripCap];
+    __shared__ uint32_t s_seam[kSeamLinks];
     __shared__ uint16_t s_r16[kTile][4];
     __shared__ uint16_t s_bottom[4];
     __shared__ uint32_t s_right[2];
-    __shared__ uint32_t s_nlinks;
+    __shared__ uint32_t s_nseam;
 
     const uint32_t tid = threadIdx.x, y = tid >> 2, c = tid & 3;
+    const uint32_t lane = tid & 31u, warp = tid >> 5;
     const uint32_t L = P.L, tiles_x = L >> 6;
     const uint32_t ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
     const uint32_t X0 = tx << 6, Y0 = ty << 6;
@@ -88,7 +95,7 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
     const uint32_t i0 = (uint32_t)(row_off + gx);           // global index of my first site
 
     if (tid < 2) s_right[tid] = 0;
-    if (tid == 2) s_nlinks = 0;
+    if (tid == 2) s_nseam = 0;
 
     // -- spins: my 16 sites, the 16 below them, and the right neighbour of my last site
     const uint4 sv = *reinterpret_cast<const uint4 *>(spins + row_off + gx);
@@ -139,33 +146,48 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
     if (c == 3 && (r16 >> 15)) atomicOr(&s_right[y >> 5], 1u << (y & 31));
 
     // -- links.  Within my 16 sites a horizontal run is named by its first site (bit tricks); only
-    //    links between runs go through the shared-memory union-find.  They are first gathered in a
-    //    CTA-wide list so that the union loop below runs with all lanes busy.
+    //    links between runs go through the shared-memory union-find.  Each warp lists the links of
+    //    its strip in row order (prefix sum over the lanes, which are in row order), then unites
+    //    them 32 at a time with all lanes busy.
     const uint32_t S = (~(lr16 << 1) | 1u) & 0xFFFFu;        // bit x: site x starts a run in my segment
     {
         const bool joint = c < 3 && (r16 >> 15);             // my last site is bonded to the next segment
+        const bool seam = (y & 7u) == 7u;                    // my down bonds leave the strip
         uint32_t v = 0, Sn = 0;
         if (ld16) {
             const uint32_t rn = s_r16[y + 1][c];
             Sn = (~(rn << 1) | 1u) & 0xFFFFu;
             v = ld16 & ~(ld16 << 1 & lr16 << 1 & rn << 1);   // bit x is redundant if bit x-1 joins the same two runs
         }
-        const uint32_t n = __popc(v) + (joint ? 1u : 0u);
-        if (n) {
-            uint32_t pos = atomicAdd(&s_nlinks, n);
-            if (joint) s_links[pos++] = (base + run_start(S, 15)) | ((base + 16) << 16);
-            while (v) {
-                const uint32_t x = __ffs(v) - 1;
-                v &= v - 1;
-                s_links[pos++] = (base + run_start(S, x)) | ((base + kTile + run_start(Sn, x)) << 16);
-            }
+        const uint32_t n_strip = (seam ? 0u : (uint32_t)__popc(v)) + (joint ? 1u : 0u);
+        uint32_t incl = n_strip;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t up = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= (uint32_t)o) incl += up;
+        }
+        const uint32_t n_warp = __shfl_sync(0xFFFFFFFFu, incl, 31);
+        uint32_t pos = incl - n_strip;
+        uint32_t *mine = s_links[warp];
+        if (joint) mine[pos++] = (base + run_start(S, 15)) | ((base + 16) << 16);
+        uint32_t *dst = mine;
+        if (seam && v) { dst = s_seam; pos = atomicAdd(&s_nseam, (uint32_t)__popc(v)); }
+        while (v) {
+            const uint32_t x = __ffs(v) - 1;
+            v &= v - 1;
+            dst[pos++] = (base + run_start(S, x)) | ((base + kTile + run_start(Sn, x)) << 16);
+        }
+        __syncwarp();
+        for (uint32_t k = lane; k < n_warp; k += 32) {
+            const uint32_t e = mine[k];
+            unite_s(s_parent, e & 0xFFFFu, e >> 16);
         }
     }
     __syncthreads();
     {
-        const uint32_t n = s_nlinks;
+        const uint32_t n = s_nseam;
         for (uint32_t k = tid; k < n; k += kTileThreads) {
-            const uint32_t e = s_links[k];
+            const uint32_t e = s_seam[k];
             unite_s(s_parent, e & 0xFFFFu, e >> 16);
         }
     }
