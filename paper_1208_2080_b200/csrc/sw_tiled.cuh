@@ -47,8 +47,15 @@ __device__ __forceinline__ uint32_t find_s(volatile uint32_t *parent, uint32_t a
 __device__ __forceinline__ void unite_s(volatile uint32_t *parent, uint32_t a, uint32_t b)
 {
     while (true) {
-        a = find_s(parent, a);
-        b = find_s(parent, b);
+        // chase both ends together (the loop runs max(depth a, depth b) times, not the sum), halving as we go
+        uint32_t pa = parent[a], pb = parent[b];
+        while (pa != a || pb != b) {
+            const uint32_t ga = parent[pa], gb = parent[pb];
+            if (ga != pa) parent[a] = ga;
+            if (gb != pb) parent[b] = gb;
+            a = ga; b = gb;
+            pa = parent[a]; pb = parent[b];
+        }
         if (a == b) return;
         if (a < b) { const uint32_t s = a; a = b; b = s; }
         const uint32_t old = atomicMin(const_cast<uint32_t *>(parent) + a, b);
@@ -62,6 +69,23 @@ __device__ __forceinline__ uint32_t pack4(uint32_t eq) { return ((eq & 0x0101010
 
 // position of the run start (highest set bit of S at or below x)
 __device__ __forceinline__ uint32_t run_start(uint32_t S, uint32_t x) { return 31u - __clz(S & ((2u << x) - 1u)); }
+
+// A link is named by the thread (y = t/4, c = t%4) that found it and the column x inside its segment:
+// vertical link = (run of site x in row y) -- (run of site x in row y+1); joint = (run of site 15) -- (first
+// site of the next segment).  The run starts are recomputed here from the shared right-bond masks, so the
+// (divergent) gather loop stays tiny and the bit tricks run with all lanes busy.
+__device__ __forceinline__ void unite_link(volatile uint32_t *parent, const uint16_t (*r16)[4], uint32_t e)
+{
+    const uint32_t t = (e >> 4) & 0xFFu, x = e & 15u;
+    const uint32_t yy = t >> 2, cc = t & 3u, base = (yy << 6) + (cc << 4);
+    const uint32_t S = (~((uint32_t)r16[yy][cc] << 1) | 1u) & 0xFFFFu;
+    uint32_t a = base + run_start(S, (e & 0x1000u) ? 15u : x), b = base + 16;
+    if (!(e & 0x1000u)) {
+        const uint32_t Sn = (~((uint32_t)r16[yy + 1][cc] << 1) | 1u) & 0xFFFFu;
+        b = base + kTile + run_start(Sn, x);
+    }
+    unite_s(parent, a, b);
+}
 
 // ---- kernel 1: bonds + tile-local labels --------------------------------------------------------
 
@@ -78,8 +102,8 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
                    TileBorder *__restrict__ border, Params P)
 {
     __shared__ uint32_t s_parent[kTileSites];
-    __shared__ uint32_t s_links[kTileThreads / 32][kStripCap];
-    __shared__ uint32_t s_seam[kSeamLinks];
+    __shared__ uint16_t s_links[kTileThreads / 32][kStripCap];   // entry: thread << 4 | x, bit 12 = segment joint
+    __shared__ uint16_t s_seam[kSeamLinks];
     __shared__ uint16_t s_r16[kTile][4];
     __shared__ uint16_t s_bottom[4];
     __shared__ uint32_t s_right[2];
@@ -153,10 +177,9 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
     {
         const bool joint = c < 3 && (r16 >> 15);             // my last site is bonded to the next segment
         const bool seam = (y & 7u) == 7u;                    // my down bonds leave the strip
-        uint32_t v = 0, Sn = 0;
+        uint32_t v = 0;
         if (ld16) {
             const uint32_t rn = s_r16[y + 1][c];
-            Sn = (~(rn << 1) | 1u) & 0xFFFFu;
             v = ld16 & ~(ld16 << 1 & lr16 << 1 & rn << 1);   // bit x is redundant if bit x-1 joins the same two runs
         }
         const uint32_t n_strip = (seam ? 0u : (uint32_t)__popc(v)) + (joint ? 1u : 0u);
@@ -168,28 +191,21 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
         }
         const uint32_t n_warp = __shfl_sync(0xFFFFFFFFu, incl, 31);
         uint32_t pos = incl - n_strip;
-        uint32_t *mine = s_links[warp];
-        if (joint) mine[pos++] = (base + run_start(S, 15)) | ((base + 16) << 16);
-        uint32_t *dst = mine;
+        uint16_t *mine = s_links[warp];
+        if (joint) mine[pos++] = (uint16_t)(0x1000u | (tid << 4));
+        uint16_t *dst = mine;
         if (seam && v) { dst = s_seam; pos = atomicAdd(&s_nseam, (uint32_t)__popc(v)); }
         while (v) {
-            const uint32_t x = __ffs(v) - 1;
+            dst[pos++] = (uint16_t)((tid << 4) | (__ffs(v) - 1));
             v &= v - 1;
-            dst[pos++] = (base + run_start(S, x)) | ((base + kTile + run_start(Sn, x)) << 16);
         }
         __syncwarp();
-        for (uint32_t k = lane; k < n_warp; k += 32) {
-            const uint32_t e = mine[k];
-            unite_s(s_parent, e & 0xFFFFu, e >> 16);
-        }
+        for (uint32_t k = lane; k < n_warp; k += 32) unite_link(s_parent, s_r16, mine[k]);
     }
     __syncthreads();
     {
         const uint32_t n = s_nseam;
-        for (uint32_t k = tid; k < n; k += kTileThreads) {
-            const uint32_t e = s_seam[k];
-            unite_s(s_parent, e & 0xFFFFu, e >> 16);
-        }
+        for (uint32_t k = tid; k < n; k += kTileThreads) unite_link(s_parent, s_r16, s_seam[k]);
     }
     __syncthreads();
 
