@@ -165,6 +165,7 @@ def run_gpu(args):
     import torch
     import torch.distributed as dist
 
+    from paper_1208_2080_b200 import replicas
     from paper_1208_2080_b200.binding import FLAG_DEFAULT, FLAG_LAZY_LABELS, SwendsenWang
 
     rank, local_rank, world = rank_info()
@@ -179,7 +180,7 @@ def run_gpu(args):
     L, q, K = c["L"], c["q"], c["K"]
     N = L * L
     flags = FLAG_LAZY_LABELS if args.lazy else FLAG_DEFAULT
-    sim = SwendsenWang(L, q, K, c["seed"] + rank, flags=flags)
+    sim = SwendsenWang(L, q, K, replicas.replica_seed(c["seed"], rank), flags=flags)
     sim.init(c["start"])
     sim.sweep(args.warmup)
     sim.synchronize()
@@ -210,11 +211,10 @@ def run_gpu(args):
     elapsed_ms = ev0.elapsed_time(ev1)
     launches = sim.stats()["kernel_launches"] - launches0
     clocks = sampler.stop(wall0, wall1) if rank == 0 else None
-    if distributed:
-        tmax = torch.tensor([elapsed_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        elapsed_ms = float(tmax.item())
-    value = world * N * args.steps / (elapsed_ms * 1e-3) / 1e9
+    # replicas only: total units of all ranks over the slowest rank's device time
+    total_units, elapsed_s, rate = replicas.aggregate_throughput(N * args.steps, elapsed_ms * 1e-3, device="cuda")
+    elapsed_ms = elapsed_s * 1e3
+    value = rate / 1e9
 
     if not per_kernel_in_region:                   # small lattice: separate pass for the per-kernel split
         sim.profile_begin()
@@ -247,11 +247,7 @@ def run_gpu(args):
         sim.get_spins_ptr(host.data_ptr())                 # D2H; synchronises
     barrier()
     e2e_s = time.perf_counter() - w0
-    if distributed:
-        tmax = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        e2e_s = float(tmax.item())
-    e2e_value = world * N * e2e_steps / e2e_s / 1e9
+    e2e_value = replicas.aggregate_throughput(N * e2e_steps, e2e_s, device="cuda")[2] / 1e9
 
     stats = sim.stats()
     if rank != 0:

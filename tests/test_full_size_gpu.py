@@ -1,0 +1,139 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (torch workspace,
+default flags, tiled path) -- needs a B200, `-m gpu`.
+
+L = 8192 / 16384: one complete sweep is compared bit for bit with the oracle (it finishes in seconds
+to a minute there).  L = 65536 (2^32 sites): the oracle needs ~10 minutes per sweep, so the default test
+checks (a) sampled outputs the oracle computes one by one -- bond draws, new states from the root's key --
+and (b) properties that hold at any size and pin the rest: every label is a fixed-point root <= the site,
+an active bond joins equal labels, no bond joins different spins, all members of a label carry the
+root's state, and the observables equal a plain numpy count over the whole lattice.  The complete
+single-step comparison with the oracle at L = 65536 is `test_L65536_full_transition_vs_oracle`
+(opt-in: SW_RUN_HUGE=1; its last recorded run is in DESIGN.md).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import binding as orc
+from oracle.binding import Oracle
+from paper_1208_2080_b200 import workloads as wl
+from paper_1208_2080_b200.binding import SwendsenWang
+
+pytestmark = pytest.mark.gpu
+
+
+def full_compare(gpu, cpu, what):
+    assert np.array_equal(gpu.get_bonds(), cpu.get_bonds()), f"bonds {what}"
+    assert np.array_equal(gpu.get_labels(), cpu.get_labels()), f"labels {what}"
+    assert np.array_equal(gpu.get_spins(), cpu.get_spins()), f"spins {what}"
+    assert gpu.measure() == cpu.measure(), f"observables {what}"
+
+
+@pytest.mark.parametrize("name", ["c3_L8192_q3", "c3_L8192_q4", "c4_L16384_q10_above"])
+def test_configs_3_and_4_one_full_sweep_vs_oracle(name):
+    c = wl.CONFIGS[name]
+    gpu = SwendsenWang(c["L"], c["q"], c["K"], c["seed"])
+    cpu = Oracle(c["L"], c["q"], c["K"], c["seed"])
+    gpu.init(c["start"]); cpu.init(c["start"])
+    gpu.sweep(1); cpu.sweep(1)
+    full_compare(gpu, cpu, name)
+
+
+def check_band(sim, pre_band, y0, h, t, rng, n_samples):
+    """Checks on rows y0 .. y0+h-1 after the sweep with counter t; pre_band = spins of rows y0 .. y0+h BEFORE it."""
+    L, q, seed = sim.L, sim.q, sim.seed
+    T = sim.get_threshold()
+    bonds = sim.get_rows("bonds", y0, h)
+    labels = np.concatenate([sim.get_rows("labels", y0, h), sim.get_rows("labels", (y0 + h) % L, 1)])
+    post = sim.get_rows("spins", y0, h)
+    pre, pre_dn = pre_band[:h], pre_band[1:h + 1]
+    eq_r = pre == np.roll(pre, -1, axis=1)
+    eq_d = pre == pre_dn
+    r, d = (bonds & 1) != 0, (bonds & 2) != 0
+    assert not np.any(r & ~eq_r) and not np.any(d & ~eq_d), "a bond joins different spins"
+    lab = labels[:h]
+    idx = (np.arange(y0, y0 + h, dtype=np.int64)[:, None] * L + np.arange(L, dtype=np.int64)[None, :])
+    assert np.all(lab.astype(np.int64) <= idx), "label above the site index"
+    assert np.array_equal(lab[r], np.roll(lab, -1, axis=1)[r]), "active right bond between different labels"
+    assert np.array_equal(lab[d], labels[1:h + 1][d]), "active down bond between different labels"
+    # bond fractions: P(active | equal) = T / 2^32
+    frac = (np.count_nonzero(r) + np.count_nonzero(d)) / max(1, np.count_nonzero(eq_r) + np.count_nonzero(eq_d))
+    assert abs(frac - T / 2.0 ** 32) < 5.0 / np.sqrt(np.count_nonzero(eq_r) + np.count_nonzero(eq_d))
+    # sampled sites, one by one through the oracle's pinned pieces
+    ys = rng.integers(0, h, n_samples); xs = rng.integers(0, L, n_samples)
+    roots = set()
+    for yy, xx in zip(ys.tolist(), xs.tolist()):
+        i = (y0 + yy) * L + xx
+        want_r = bool(eq_r[yy, xx]) and orc.draw_bond(seed, t, i, 0) < T
+        want_d = bool(eq_d[yy, xx]) and orc.draw_bond(seed, t, i, 1) < T
+        assert (bool(r[yy, xx]), bool(d[yy, xx])) == (want_r, want_d), f"bond at site {i}"
+        root = int(lab[yy, xx])
+        assert int(post[yy, xx]) == orc.state_from_draw(orc.draw_flip(seed, t, root), q), f"new state at site {i}"
+        roots.add(root)
+    # sampled labels are fixed-point roots: labels[root] == root (fetched row by row)
+    for root in list(roots)[:64]:
+        ry, rx = divmod(root, L)
+        assert int(sim.get_rows("labels", ry, 1)[0, rx]) == root, f"label {root} is not a root"
+
+
+@pytest.mark.parametrize("name", ["c5_L65536_q2", "c4_L16384_q10_below", "c2_L4096_q2"])
+def test_full_size_properties_and_sampled_outputs(name):
+    c = wl.CONFIGS[name]
+    L, q = c["L"], c["q"]
+    N = L * L
+    rng = np.random.default_rng(42)
+    sim = SwendsenWang(L, q, c["K"], c["seed"])
+    sim.init(c["start"])
+    sim.sweep(2)
+    t = sim.get_time()
+    h = 192 if L >= 192 else L - 1
+    bands = [0, 63, L // 2 - 70, L - h - 1][: (4 if L > 1024 else 2)]          # bands straddle tile rows
+    pre = {y0: sim.get_rows("spins", y0, h + 1) for y0 in bands}
+    pre_first = sim.get_rows("spins", 0, 1)
+    pre_last = sim.get_rows("spins", L - 64, 64)
+    sim.sweep(1)
+    for y0 in bands:
+        check_band(sim, pre[y0], y0, h, t, rng, 300)
+    # the periodic seam: last 64 rows, whose down neighbours are row 0
+    check_band(sim, np.concatenate([pre_last, pre_first]), L - 64, 64, t, rng, 200)
+
+    # observables against plain numpy counts over the whole lattice, in row chunks
+    m = sim.measure()
+    rows = max(1, min(L, (1 << 28) // L))
+    e = 0
+    mag = np.zeros(q, dtype=np.int64)
+    n_roots = 0
+    first_row = sim.get_rows("spins", 0, 1)
+    for y0 in range(0, L, rows):
+        nr = min(rows, L - y0)
+        s = sim.get_rows("spins", y0, nr)
+        nxt = sim.get_rows("spins", y0 + nr, 1) if y0 + nr < L else first_row
+        e += int(np.count_nonzero(s[:, :-1] == s[:, 1:])) + int(np.count_nonzero(s[:, -1] == s[:, 0]))
+        e += int(np.count_nonzero(s[:-1] == s[1:])) + int(np.count_nonzero(s[-1] == nxt[0]))
+        mag += np.bincount(s.reshape(-1), minlength=q)
+        del s
+        lab = sim.get_rows("labels", y0, nr).reshape(-1)
+        n_roots += int(np.count_nonzero(lab == np.arange(y0 * L, (y0 + nr) * L, dtype=np.uint32)))
+        del lab
+    assert m["energy_bonds"] == e
+    assert m["mag_counts"] == mag.tolist() and int(mag.sum()) == N
+    assert m["n_clusters"] == n_roots
+    assert 1 <= m["largest_cluster"] <= N
+
+
+@pytest.mark.huge
+@pytest.mark.skipif(os.environ.get("SW_RUN_HUGE") != "1", reason="~15 min of host CPU and ~35 GiB of host RAM; set SW_RUN_HUGE=1")
+def test_L65536_full_transition_vs_oracle():
+    """Single-step transition check: GPU spins after sweep t-1 are handed to the oracle,
+    one oracle sweep, everything compared with the GPU's sweep t.  t = 1 and a late t."""
+    c = wl.CONFIGS["c5_L65536_q2"]
+    gpu = SwendsenWang(c["L"], c["q"], c["K"], c["seed"])
+    cpu = Oracle(c["L"], c["q"], c["K"], c["seed"])
+    gpu.init(c["start"])
+    for warm in (1, int(os.environ.get("SW_HUGE_LATE_T", "40"))):
+        gpu.sweep(warm - gpu.get_time())
+        t = gpu.get_time()
+        cpu.set_state(gpu.get_spins(), t)
+        gpu.sweep(1); cpu.sweep(1)
+        full_compare(gpu, cpu, f"L=65536 sweep {t}")
