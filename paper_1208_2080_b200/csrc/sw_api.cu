@@ -155,7 +155,10 @@ int sweep_once(sw_ctx *c)
         { Timed tm(c, SLOT_MERGE);
           sw::k_tile_merge<<<tiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, P); }
         { Timed tm(c, SLOT_FLIP);
-          sw::k_tile_flip<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->lazy ? 0 : 1); }
+          if (P.log2L != 0xFFFFFFFFu)
+              sw::k_tile_flip<true><<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->lazy ? 0 : 1);
+          else
+              sw::k_tile_flip<false><<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->lazy ? 0 : 1); }
         c->labels_flat = !c->lazy;
     } else {
         const int th = 256;

@@ -291,16 +291,17 @@ k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, Params P)
 // distinct root seen by the tile is chased and drawn ONCE (work spread over the whole CTA) and
 // every other site needs one shared-memory lookup.
 
+template <bool kPow2>
 __global__ void __launch_bounds__(kTileThreads)
 k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__restrict__ spins,
             Params P, int write_labels)
 {
     __shared__ uint32_t s_root[kTileSites];                   // per tile-local root: its canonical root
     __shared__ uint8_t s_state[kTileSites];                   // per tile-local root: the new state
-    __shared__ uint16_t s_list[kTileSites];
-    __shared__ uint32_t s_count;
+    __shared__ uint16_t s_list[kTileThreads / 32][512];       // per warp: the tile-local roots of its 8 rows
 
     const uint32_t tid = threadIdx.x, y = tid >> 2, c = tid & 3;
+    const uint32_t lane = tid & 31u, warp = tid >> 5;
     const uint32_t L = P.L, tiles_x = L >> 6;
     const uint32_t ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
     const uint32_t X0 = tx << 6, Y0 = ty << 6;
@@ -310,9 +311,37 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
     const uint32_t origin = Y0 * L + X0;
     const uint32_t base = (y << 6) + (c << 4);
 
-    if (tid == 0) s_count = 0;
+    // -- phase A: each warp lists the tile-local roots of its strip (prefix sum over the lanes, no atomics)
+    const uint32_t work = rootbits[i0 >> 4];
+    uint32_t n_warp;
+    {
+        const uint32_t n = __popc(work);
+        uint32_t incl = n;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t up = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= (uint32_t)o) incl += up;
+        }
+        n_warp = __shfl_sync(0xFFFFFFFFu, incl, 31);
+        uint32_t pos = incl - n, m = work;
+        while (m) {
+            s_list[warp][pos++] = (uint16_t)(base + __ffs(m) - 1);
+            m &= m - 1;
+        }
+    }
+    __syncwarp();
 
-    // -- phase A: my 16 labels; queue the tile-local roots among them
+    // -- phase B: one chase + one Philox call per tile-local root, 32 at a time per warp
+    for (uint32_t k = lane; k < n_warp; k += 32) {
+        const uint32_t id = s_list[warp][k];
+        const uint32_t self = origin + (id >> 6) * L + (id & 63u);
+        const uint32_t g = find_root(labels, self);
+        s_root[id] = g;
+        s_state[id] = (uint8_t)flip_state(g, P);
+    }
+    __syncthreads();
+
+    // -- phase C: every site looks its tile-local root up; consecutive sites with the same label share a lookup
     uint32_t lab[16];
     {
         const uint4 *lp = reinterpret_cast<const uint4 *>(labels + row_off + gx);
@@ -322,41 +351,21 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
             lab[4 * k] = l.x; lab[4 * k + 1] = l.y; lab[4 * k + 2] = l.z; lab[4 * k + 3] = l.w;
         }
     }
-    const uint32_t work = rootbits[i0 >> 4];
-    __syncthreads();
-    if (work) {
-        uint32_t pos = atomicAdd(&s_count, (uint32_t)__popc(work));
-#pragma unroll
-        for (int j = 0; j < 16; ++j) {
-            if ((work >> j) & 1u) {
-                s_root[base + j] = lab[j];
-                s_list[pos++] = (uint16_t)(base + j);
-            }
-        }
-    }
-    __syncthreads();
-
-    // -- phase B: one chase + one Philox call per tile-local root
-    const uint32_t count = s_count;
-    for (uint32_t k = tid; k < count; k += kTileThreads) {
-        const uint32_t id = s_list[k];
-        const uint32_t l = s_root[id];
-        const uint32_t self = origin + (id >> 6) * L + (id & 63u);
-        const uint32_t g = (l == self) ? l : find_root(labels, l);
-        s_root[id] = g;
-        s_state[id] = (uint8_t)flip_state(g, P);
-    }
-    __syncthreads();
-
-    // -- phase C: every site looks its tile-local root up
     uint32_t st[4] = {0, 0, 0, 0};
+    uint32_t prev = 0, root = 0, state = 0;
 #pragma unroll
     for (int j = 0; j < 16; ++j) {
-        const uint32_t d = (((work >> j) & 1u) ? i0 + j : lab[j]) - origin;
-        const uint32_t dy = div_L(d, P);
-        const uint32_t id = (dy << 6) + (d - dy * L);
-        lab[j] = s_root[id];
-        st[j >> 2] |= (uint32_t)s_state[id] << (8 * (j & 3));
+        const uint32_t le = ((work >> j) & 1u) ? i0 + j : lab[j];   // a tile-local root stands for itself
+        if (j == 0 || le != prev) {
+            const uint32_t d = le - origin;
+            const uint32_t dy = kPow2 ? (d >> P.log2L) : (uint32_t)(((uint64_t)d * P.divL_magic) >> 40);
+            const uint32_t id = (dy << 6) + (d - dy * L);
+            root = s_root[id];
+            state = s_state[id];
+            prev = le;
+        }
+        lab[j] = root;
+        st[j >> 2] |= state << (8 * (j & 3));
     }
     *reinterpret_cast<uint4 *>(spins + row_off + gx) = make_uint4(st[0], st[1], st[2], st[3]);
     if (write_labels) {
