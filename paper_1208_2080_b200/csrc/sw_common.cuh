@@ -68,14 +68,32 @@ __device__ __forceinline__ uint32_t find_root(const uint32_t *labels, uint32_t a
     return a;
 }
 
+// find with path halving: every second node on the way is re-pointed at its grandparent.  A link is
+// only ever replaced by a link to an ancestor, so this is safe next to concurrent hooks (a hook that
+// loses the race sees the old value come back from atomicMin and carries on from there).  The
+// re-pointing is itself an atomicMin (a fire-and-forget RED): it can only lower a link, so it can
+// never undo a canonical root that k_tile_flip of another tile has already written there.
+__device__ __forceinline__ uint32_t find_root_halving(uint32_t *labels, uint32_t a)
+{
+    uint32_t p = ld_label(labels, a);
+    while (p != a) {
+        const uint32_t gp = ld_label(labels, p);
+        if (gp == p) return p;
+        atomicMin(labels + a, gp);
+        a = gp;
+        p = ld_label(labels, a);
+    }
+    return a;
+}
+
 // Join the sets of a and b.  The larger root is hooked under the smaller with atomicMin; if the
 // word we hit was no longer a root, the link it held is not lost: we carry on uniting its old
 // target with b.  One pass over all bonds yields the complete partition (no outer iteration).
 __device__ __forceinline__ void unite(uint32_t *labels, uint32_t a, uint32_t b)
 {
     while (true) {
-        a = find_root(labels, a);
-        b = find_root(labels, b);
+        a = find_root_halving(labels, a);
+        b = find_root_halving(labels, b);
         if (a == b) return;
         if (a < b) { const uint32_t s = a; a = b; b = s; }
         const uint32_t old = atomicMin(labels + a, b);

@@ -335,7 +335,7 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
     for (uint32_t k = lane; k < n_warp; k += 32) {
         const uint32_t id = s_list[warp][k];
         const uint32_t self = origin + (id >> 6) * L + (id & 63u);
-        const uint32_t g = find_root(labels, self);
+        const uint32_t g = find_root_halving(labels, self);
         s_root[id] = g;
         s_state[id] = (uint8_t)flip_state(g, P);
     }
