@@ -27,22 +27,17 @@ struct __align__(16) TileBorder {
 };
 
 // ---- shared-memory union-find (tile-local) -----------------------------------------------------
-// Links always point to a smaller local id, so plain stores that replace a link by a link to an
-// ancestor (path halving) are safe next to concurrent atomicMin hooks: nothing that was joined
-// can come apart, and the root of a set is always its smallest member.
+// Nodes are "pieces": maximal runs of right-bonded sites inside one thread's 16-site segment, named
+// by their first site.  A node id is the PADDED local index 17 * thread + x (one spare word per 16
+// entries, so that the 32 lanes of a warp, which own segments 16 words apart, fall in 32 different
+// banks).  Padding keeps the row-major order, so "smaller id" still means "smaller site index".
+//
+// Links always point to a smaller id, so plain stores that replace a link by a link to an ancestor
+// (path halving) are safe next to concurrent atomicMin hooks: nothing that was joined can come
+// apart, and the root of a set is always its smallest member ("proper label").
 
-__device__ __forceinline__ uint32_t find_s(volatile uint32_t *parent, uint32_t a)
-{
-    uint32_t p = parent[a];
-    while (p != a) {
-        const uint32_t gp = parent[p];
-        if (gp == p) return p;
-        parent[a] = gp;                                   // path halving
-        a = gp;
-        p = parent[a];
-    }
-    return a;
-}
+constexpr uint32_t kPad = 17;                               // padded words per 16-site segment
+constexpr uint32_t kParentWords = kTileThreads * kPad;      // 4352
 
 __device__ __forceinline__ void unite_s(volatile uint32_t *parent, uint32_t a, uint32_t b)
 {
@@ -67,47 +62,53 @@ __device__ __forceinline__ void unite_s(volatile uint32_t *parent, uint32_t a, u
 // the four 0x00/0xFF bytes of a __vcmpeq4 result -> 4 bits
 __device__ __forceinline__ uint32_t pack4(uint32_t eq) { return ((eq & 0x01010101u) * 0x01020408u) >> 24; }
 
-// position of the run start (highest set bit of S at or below x)
+// position of the piece start (highest set bit of S at or below x)
 __device__ __forceinline__ uint32_t run_start(uint32_t S, uint32_t x) { return 31u - __clz(S & ((2u << x) - 1u)); }
 
-// A link is named by the thread (y = t/4, c = t%4) that found it and the column x inside its segment:
-// vertical link = (run of site x in row y) -- (run of site x in row y+1); joint = (run of site 15) -- (first
-// site of the next segment).  The run starts are recomputed here from the shared right-bond masks, so the
-// (divergent) gather loop stays tiny and the bit tricks run with all lanes busy.
-__device__ __forceinline__ void unite_link(volatile uint32_t *parent, const uint16_t (*r16)[4], uint32_t e)
+// piece-start mask of a segment from its (tile-local) right-bond mask: site x starts a piece unless bonded to x-1
+__device__ __forceinline__ uint32_t starts_of(uint32_t r16) { return (~(r16 << 1) | 1u) & 0xFFFFu; }
+
+// An extra link is named by the thread t = 4y + c that owns its LOWER end and a column x of its segment:
+// vertical = (piece of site x in row y) -- (piece of site x in row y-1); joint (bit 12) = (first piece of the
+// segment) -- (last piece of the segment to its left).  The piece starts are recomputed from the shared
+// bond masks, so the list entry stays 16 bits.
+__device__ __forceinline__ void unite_link(volatile uint32_t *parent, const uint32_t *rd, uint32_t e)
 {
     const uint32_t t = (e >> 4) & 0xFFu, x = e & 15u;
-    const uint32_t yy = t >> 2, cc = t & 3u, base = (yy << 6) + (cc << 4);
-    const uint32_t S = (~((uint32_t)r16[yy][cc] << 1) | 1u) & 0xFFFFu;
-    uint32_t a = base + run_start(S, (e & 0x1000u) ? 15u : x), b = base + 16;
-    if (!(e & 0x1000u)) {
-        const uint32_t Sn = (~((uint32_t)r16[yy + 1][cc] << 1) | 1u) & 0xFFFFu;
-        b = base + kTile + run_start(Sn, x);
+    uint32_t a, b;
+    if (e & 0x1000u) {
+        a = t * kPad;
+        b = (t - 1) * kPad + run_start(starts_of(rd[t - 1] & 0xFFFFu), 15u);
+    } else {
+        a = t * kPad + run_start(starts_of(rd[t] & 0xFFFFu), x);
+        b = (t - 4) * kPad + run_start(starts_of(rd[t - 4] & 0xFFFFu), x);
     }
     unite_s(parent, a, b);
 }
 
 // ---- kernel 1: bonds + tile-local labels --------------------------------------------------------
+// Labeling in four phases (the idea of label equivalence without the outer iteration: one
+// assignment pass, one pass over the leftover equivalences, one resolve pass):
+//   A  every piece that has a neighbour piece above it (or to its left, across a segment joint)
+//      takes ONE of them as its parent with a plain store: no search, no atomics.  Parents have
+//      smaller ids, so this is a forest.
+//   B  the remaining links (second and later up-links of a piece, up-links of a piece that took its
+//      joint) are real equivalences: united with find + atomicMin, 32 at a time per warp.
+//   C  every piece is pointed straight at its root.  A warp walks the pieces of its 8-row strip in
+//      row order, so the parent of a piece is almost always resolved already (as in the second
+//      pass of a sequential Hoshen-Kopelman labeling).
+//   D  each thread reads the roots of its pieces and writes labels, root flags and the border record.
+constexpr uint32_t kListCap = 8 * 64 + 32;             // pieces of a strip <= 512; extra links of a strip <= 512 + 24
 
-// A warp owns the 8 tile rows 8w .. 8w+7 (its "strip").  Links inside a strip are united by that
-// warp alone, in row order (which keeps the trees shallow, as in a sequential Hoshen-Kopelman
-// sweep); the links between strips are united by the whole CTA afterwards.
-constexpr uint32_t kStripLinks = 7 * 64 + 8 * 3;      // vertical bonds inside a strip + its segment joints = 472
-constexpr uint32_t kStripCap = 480;
-constexpr uint32_t kSeamLinks = 7 * 64;               // vertical bonds between strips
-
-__global__ void __launch_bounds__(kTileThreads)
+__global__ void __launch_bounds__(kTileThreads, 8)
 k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
                    uint32_t *__restrict__ labels, uint16_t *__restrict__ rootbits,
                    TileBorder *__restrict__ border, Params P)
 {
-    __shared__ uint32_t s_parent[kTileSites];
-    __shared__ uint16_t s_links[kTileThreads / 32][kStripCap];   // entry: thread << 4 | x, bit 12 = segment joint
-    __shared__ uint16_t s_seam[kSeamLinks];
-    __shared__ uint16_t s_r16[kTile][4];
-    __shared__ uint16_t s_bottom[4];
+    __shared__ uint32_t s_parent[kParentWords];
+    __shared__ uint32_t s_rd[kTileThreads];                    // per thread: tile-local right bonds | down bonds << 16
+    __shared__ uint16_t s_list[kTileThreads / 32][kListCap];   // per warp: extra links (phase B), then pieces (phase C)
     __shared__ uint32_t s_right[2];
-    __shared__ uint32_t s_nseam;
 
     const uint32_t tid = threadIdx.x, y = tid >> 2, c = tid & 3;
     const uint32_t lane = tid & 31u, warp = tid >> 5;
@@ -119,7 +120,6 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
     const uint32_t i0 = (uint32_t)(row_off + gx);           // global index of my first site
 
     if (tid < 2) s_right[tid] = 0;
-    if (tid == 2) s_nseam = 0;
 
     // -- spins: my 16 sites, the 16 below them, and the right neighbour of my last site
     const uint4 sv = *reinterpret_cast<const uint4 *>(spins + row_off + gx);
@@ -155,91 +155,120 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
 
     // -- tile-local masks: bonds that leave the tile are recorded in the border record instead
     const uint32_t lr16 = (c == 3) ? (r16 & 0x7FFFu) : r16;
-    const uint32_t ld16 = (y == kTile - 1) ? 0u : d16;
-    s_r16[y][c] = (uint16_t)lr16;
-    if (y == kTile - 1) s_bottom[c] = (uint16_t)d16;
-    const uint32_t base = (y << 6) + (c << 4);               // local id of my first site
-    {
-        uint4 *pp = reinterpret_cast<uint4 *>(s_parent + base);
-        pp[0] = make_uint4(base + 0, base + 1, base + 2, base + 3);
-        pp[1] = make_uint4(base + 4, base + 5, base + 6, base + 7);
-        pp[2] = make_uint4(base + 8, base + 9, base + 10, base + 11);
-        pp[3] = make_uint4(base + 12, base + 13, base + 14, base + 15);
-    }
+    s_rd[tid] = lr16 | (d16 << 16);                           // (row 63's down bonds are only read for the border record)
+    const uint32_t pbase = tid * kPad;                       // padded id of my first site
+    const uint32_t S = starts_of(lr16);                      // bit x: site x starts a piece
+#pragma unroll
+    for (int x = 0; x < 16; ++x)
+        if ((S >> x) & 1u) s_parent[pbase + x] = pbase + x;
     __syncthreads();
     if (c == 3 && (r16 >> 15)) atomicOr(&s_right[y >> 5], 1u << (y & 31));
 
-    // -- links.  Within my 16 sites a horizontal run is named by its first site (bit tricks); only
-    //    links between runs go through the shared-memory union-find.  Each warp lists the links of
-    //    its strip in row order (prefix sum over the lanes, which are in row order), then unites
-    //    them 32 at a time with all lanes busy.
-    const uint32_t S = (~(lr16 << 1) | 1u) & 0xFFFFu;        // bit x: site x starts a run in my segment
+    // -- phase A: one parent per piece, by plain store
+    const uint32_t C = S ^ 0xFFFFu;                          // bit x: site x continues the piece of x-1
+    uint32_t extra;                                          // up-links that phase B must still unite
+    bool joint;                                              // my first piece is bonded to the segment on my left
     {
-        const bool joint = c < 3 && (r16 >> 15);             // my last site is bonded to the next segment
-        const bool seam = (y & 7u) == 7u;                    // my down bonds leave the strip
-        uint32_t v = 0;
-        if (ld16) {
-            const uint32_t rn = s_r16[y + 1][c];
-            v = ld16 & ~(ld16 << 1 & lr16 << 1 & rn << 1);   // bit x is redundant if bit x-1 joins the same two runs
+        const uint32_t up = (y > 0) ? s_rd[tid - 4] : 0u;
+        const uint32_t s = up >> 16;                          // bit x: up-link (row y-1, x) -- (row y, x)
+        const uint32_t S_up = starts_of(up & 0xFFFFu);
+        const uint32_t left = __shfl_up_sync(0xFFFFFFFFu, lr16, 1);
+        joint = c > 0 && ((left >> 15) & 1u);
+        // first up-link of every piece: carry chain with generate = s, propagate = C gives, for every
+        // site, "some up-link at a smaller x of my piece"
+        const uint32_t A = s | C;
+        const uint32_t cin = (A + s) ^ A ^ s;                 // bit x: carry into x
+        uint32_t first = s & ~(cin & C);
+        // an up-link whose left neighbour is an up-link between the same two pieces says nothing new
+        const uint32_t v = s & ~((s << 1) & C & ~S_up);
+        if (joint) {
+            const uint32_t second = S & (S - 1u);             // piece starts after the first one
+            const uint32_t e0 = (second & (0u - second)) - 1u;   // extent of my first piece (all ones if it is the only one)
+            first &= ~e0;                                     // that piece takes the joint; its up-links become extras
+            s_parent[pbase] = pbase - kPad + run_start(starts_of(left & 0xFFFFu), 15u);
         }
-        const uint32_t n_strip = (seam ? 0u : (uint32_t)__popc(v)) + (joint ? 1u : 0u);
-        uint32_t incl = n_strip;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t up = __shfl_up_sync(0xFFFFFFFFu, incl, o);
-            if (lane >= (uint32_t)o) incl += up;
+        extra = v & ~first;
+        while (first) {
+            const uint32_t x = __ffs(first) - 1;
+            first &= first - 1;
+            s_parent[pbase + run_start(S, x)] = pbase - 4 * kPad + run_start(S_up, x);
         }
-        const uint32_t n_warp = __shfl_sync(0xFFFFFFFFu, incl, 31);
-        uint32_t pos = incl - n_strip;
-        uint16_t *mine = s_links[warp];
-        if (joint) mine[pos++] = (uint16_t)(0x1000u | (tid << 4));
-        uint16_t *dst = mine;
-        if (seam && v) { dst = s_seam; pos = atomicAdd(&s_nseam, (uint32_t)__popc(v)); }
-        while (v) {
-            dst[pos++] = (uint16_t)((tid << 4) | (__ffs(v) - 1));
-            v &= v - 1;
-        }
-        __syncwarp();
-        for (uint32_t k = lane; k < n_warp; k += 32) unite_link(s_parent, s_r16, mine[k]);
     }
     __syncthreads();
+
+    // -- phase B: the remaining links, gathered per warp (prefix sum over the lanes) and united 32 at a time
     {
-        const uint32_t n = s_nseam;
-        for (uint32_t k = tid; k < n; k += kTileThreads) unite_link(s_parent, s_r16, s_seam[k]);
+        const uint32_t n = (uint32_t)__popc(extra);
+        uint32_t incl = n;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t upv = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= (uint32_t)o) incl += upv;
+        }
+        const uint32_t n_warp = __shfl_sync(0xFFFFFFFFu, incl, 31);
+        uint32_t pos = incl - n;
+        uint16_t *mine = s_list[warp];
+        while (extra) {
+            mine[pos++] = (uint16_t)((tid << 4) | (__ffs(extra) - 1));
+            extra &= extra - 1;
+        }
+        __syncwarp();
+        for (uint32_t k = lane; k < n_warp; k += 32) unite_link(s_parent, s_rd, mine[k]);
     }
     __syncthreads();
 
     if (tid == 0) {
         TileBorder b;
         b.right_col = (unsigned long long)s_right[0] | ((unsigned long long)s_right[1] << 32);
-        b.bottom_row = (unsigned long long)s_bottom[0] | ((unsigned long long)s_bottom[1] << 16) |
-                       ((unsigned long long)s_bottom[2] << 32) | ((unsigned long long)s_bottom[3] << 48);
+        b.bottom_row = (unsigned long long)(s_rd[252] >> 16) | ((unsigned long long)(s_rd[253] >> 16) << 16) |
+                       ((unsigned long long)(s_rd[254] >> 16) << 32) | ((unsigned long long)(s_rd[255] >> 16) << 48);
         border[blockIdx.x] = b;
     }
 
-    // -- compress: every entry points straight at its root (no hooks happen any more)
-#pragma unroll 4
-    for (uint32_t j = 0; j < 16; ++j) {
-        const uint32_t id = tid + j * kTileThreads;
-        const uint32_t p = s_parent[id];
-        if (p != id) {                                       // read-only chase: other threads finalise entries now
-            uint32_t r = p, g = const_cast<volatile uint32_t *>(s_parent)[r];
-            while (g != r) { r = g; g = const_cast<volatile uint32_t *>(s_parent)[r]; }
-            if (r != p) s_parent[id] = r;
+    // -- phase C: point every piece of my warp's strip at its root, in row order (no hooks happen any more)
+    {
+        const uint32_t n = (uint32_t)__popc(S);
+        uint32_t incl = n;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t upv = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= (uint32_t)o) incl += upv;
+        }
+        const uint32_t n_warp = __shfl_sync(0xFFFFFFFFu, incl, 31);
+        uint32_t pos = incl - n, m = S;
+        uint16_t *mine = s_list[warp];
+        while (m) {
+            mine[pos++] = (uint16_t)(pbase + __ffs(m) - 1);
+            m &= m - 1;
+        }
+        __syncwarp();
+        volatile uint32_t *par = s_parent;
+        for (uint32_t k0 = 0; k0 < n_warp; k0 += 32) {
+            const uint32_t k = k0 + lane;
+            if (k < n_warp) {
+                const uint32_t id = mine[k];
+                const uint32_t p = par[id];
+                if (p != id) {
+                    uint32_t r = p, g = par[r];
+                    while (g != r) { r = g; g = par[r]; }
+                    if (r != p) par[id] = r;
+                }
+            }
+            __syncwarp();
         }
     }
-    __syncthreads();
 
-    // -- labels: global index of the smallest site of my tile-local component; root flags
+    // -- phase D: labels = global index of the smallest site of my tile-local component; root flags
     const uint32_t origin = Y0 * L + X0;
     uint32_t lab[16];
     uint32_t cur = 0, roots = 0;
 #pragma unroll
     for (int x = 0; x < 16; ++x) {
         if ((S >> x) & 1u) {
-            const uint32_t r = s_parent[base + x];
-            cur = origin + (r >> 6) * L + (r & 63u);
-            roots |= (r == base + x) ? (1u << x) : 0u;
+            const uint32_t r = s_parent[pbase + x];
+            const uint32_t t = (r * 61681u) >> 20;           // r / 17 for r < 4352: the thread that owns the root
+            cur = origin + (t >> 2) * L + ((t & 3u) << 4) + (r - t * kPad);
+            roots |= (r == pbase + x) ? (1u << x) : 0u;
         }
         lab[x] = cur;
     }
