@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <new>
 #include <string>
 #include <vector>
@@ -15,6 +16,7 @@
 #include "sw_generic.cuh"
 #include "sw_observe.cuh"
 #include "sw_tiled.cuh"
+#include "sw_tile_warp.cuh"
 
 namespace {
 
@@ -30,7 +32,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Plan {
-    size_t spins, bonds, labels, rootbits, border, row, flag, total;   // byte offsets into the workspace
+    size_t spins, bonds, labels, rootbits, border, cols, row, flag, total;   // byte offsets into the workspace
 };
 
 bool tiled_ok(uint32_t L, uint32_t flags) { return (L % sw::kTile == 0) && !(flags & SW_FLAG_FORCE_GENERIC); }
@@ -45,6 +47,7 @@ Plan make_plan(uint32_t L, uint32_t q, uint32_t flags)
     p.labels = off; off = align_up(off + N * 4);
     p.rootbits = off; off = align_up(off + (tiled_ok(L, flags) ? (N / 16) * 2 : 0));
     p.border = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileBorder) : 0));
+    p.cols = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileCols) : 0));
     p.row = off;    off = align_up(off + (3 + (size_t)q) * 8);
     p.flag = off;   off = align_up(off + 4);
     p.total = off;
@@ -68,10 +71,12 @@ struct sw_ctx {
     uint32_t *d_bonds = nullptr, *d_labels = nullptr, *d_flag = nullptr;
     uint16_t *d_rootbits = nullptr;
     sw::TileBorder *d_border = nullptr;
+    sw::TileCols *d_cols = nullptr;
     unsigned long long *d_row = nullptr;
     uint32_t *d_sizes = nullptr;          // lazily allocated 4N-byte scratch for cluster sizes
     uint64_t launches = 0, sweeps = 0;
     int num_sms = 148;
+    int tile_variant = 0;                 // development switch (env SW_TILE_VARIANT): 0 = warp per tile, 1 = CTA per tile
     // profiling
     bool profiling = false;
     struct Ev { int slot; cudaEvent_t a, b; };
@@ -151,14 +156,17 @@ int sweep_once(sw_ctx *c)
     if (c->tiled) {
         const unsigned tiles = (unsigned)(c->N / sw::kTileSites);
         { Timed tm(c, SLOT_TILE);
-          sw::k_tile_bonds_label<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, P); }
+          if (c->tile_variant == 0)
+              sw::k_tile_warp<<<(tiles + sw::kTwWarps - 1) / sw::kTwWarps, sw::kTwThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_cols, P, tiles);
+          else
+              sw::k_tile_bonds_label<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_cols, P); }
         { Timed tm(c, SLOT_MERGE);
-          sw::k_tile_merge<<<tiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, P); }
+          sw::k_tile_merge<<<tiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_cols, P); }
         { Timed tm(c, SLOT_FLIP);
           if (P.log2L != 0xFFFFFFFFu)
-              sw::k_tile_flip<true><<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->lazy ? 0 : 1);
+              sw::k_tile_flip<true><<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->lazy ? 0 : 1);
           else
-              sw::k_tile_flip<false><<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->lazy ? 0 : 1); }
+              sw::k_tile_flip<false><<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->lazy ? 0 : 1); }
         c->labels_flat = !c->lazy;
     } else {
         const int th = 256;
@@ -242,6 +250,7 @@ int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed,
     cudaError_t e = cudaGetDevice(&c->device);
     if (e != cudaSuccess) { delete c; return SW_ERR_CUDA; }
     cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
+    if (const char *v = getenv("SW_TILE_VARIANT")) c->tile_variant = atoi(v);
     if (external) {
         if (!dev_ws || ws_bytes < plan.total || ((uintptr_t)dev_ws % kAlign) != 0) { delete c; return dev_ws ? SW_ERR_OOM : SW_ERR_INVALID_ARG; }
         c->ws = (uint8_t *)dev_ws; c->stream = (cudaStream_t)stream;
@@ -257,6 +266,7 @@ int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed,
     c->d_labels = (uint32_t *)(c->ws + plan.labels);
     c->d_rootbits = (uint16_t *)(c->ws + plan.rootbits);
     c->d_border = (sw::TileBorder *)(c->ws + plan.border);
+    c->d_cols = (sw::TileCols *)(c->ws + plan.cols);
     c->d_row = (unsigned long long *)(c->ws + plan.row);
     c->d_flag = (uint32_t *)(c->ws + plan.flag);
     *out = c;

@@ -86,6 +86,19 @@ __device__ __forceinline__ uint32_t find_root_halving(uint32_t *labels, uint32_t
     return a;
 }
 
+// the same chase when the caller already holds p = labels[a] (possibly stale: still an ancestor)
+__device__ __forceinline__ uint32_t find_root_halving_from(uint32_t *labels, uint32_t a, uint32_t p)
+{
+    while (p != a) {
+        const uint32_t gp = ld_label(labels, p);
+        if (gp == p) return p;
+        atomicMin(labels + a, gp);
+        a = gp;
+        p = ld_label(labels, a);
+    }
+    return a;
+}
+
 // Join the sets of a and b.  The larger root is hooked under the smaller with atomicMin; if the
 // word we hit was no longer a root, the link it held is not lost: we carry on uniting its old
 // target with b.  One pass over all bonds yields the complete partition (no outer iteration).

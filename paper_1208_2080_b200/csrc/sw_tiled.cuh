@@ -26,6 +26,13 @@ struct __align__(16) TileBorder {
     unsigned long long bottom_row;  // bit x: bond (X0+x, Y0+63) -> (X0+x, Y0+64)
 };
 
+// per-tile copy of the tile-local labels of the left and right columns (written by the tile kernel,
+// read by k_tile_merge): a column of labels[] is one 32-byte sector per site, these are 256 bytes each
+struct __align__(16) TileCols {
+    uint32_t left[kTile];           // label of site (X0,      Y0 + y)
+    uint32_t right[kTile];          // label of site (X0 + 63, Y0 + y)
+};
+
 // ---- shared-memory union-find (tile-local) -----------------------------------------------------
 // Nodes are "pieces": maximal runs of right-bonded sites inside one thread's 16-site segment, named
 // by their first site.  A node id is the PADDED local index 17 * thread + x (one spare word per 16
@@ -103,7 +110,7 @@ constexpr uint32_t kListCap = 8 * 64 + 32;             // pieces of a strip <= 5
 __global__ void __launch_bounds__(kTileThreads, 8)
 k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
                    uint32_t *__restrict__ labels, uint16_t *__restrict__ rootbits,
-                   TileBorder *__restrict__ border, Params P)
+                   TileBorder *__restrict__ border, TileCols *__restrict__ cols, Params P)
 {
     __shared__ uint32_t s_parent[kParentWords];
     __shared__ uint32_t s_rd[kTileThreads];                    // per thread: tile-local right bonds | down bonds << 16
@@ -278,34 +285,36 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
     lp[2] = make_uint4(lab[8], lab[9], lab[10], lab[11]);
     lp[3] = make_uint4(lab[12], lab[13], lab[14], lab[15]);
     rootbits[i0 >> 4] = (uint16_t)roots;
+    if (c == 0) cols[blockIdx.x].left[y] = lab[0];
+    if (c == 3) cols[blockIdx.x].right[y] = lab[15];
 }
 
 // ---- kernel 2: merge across tile borders -------------------------------------------------------
 // One CTA per tile, one thread per border site (64 on the right column, 64 on the bottom row).
 
 __global__ void __launch_bounds__(kMergeThreads)
-k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, Params P)
+k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, const TileCols *__restrict__ cols, Params P)
 {
     const uint32_t b = threadIdx.x;
     const uint32_t L = P.L, tiles_x = L >> 6;
     const uint32_t ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
     const uint32_t X0 = tx << 6, Y0 = ty << 6;
     const TileBorder rec = border[blockIdx.x];
-    uint32_t u, v;
+    const uint32_t *pu, *pv;
     unsigned long long mask;
     uint32_t k;
-    if (b < kTile) {
+    if (b < kTile) {                                         // right column -- left column of the tile on the right
         k = b; mask = rec.right_col;
-        u = (Y0 + k) * L + X0 + (kTile - 1);
-        v = (Y0 + k) * L + ((X0 + kTile == L) ? 0u : X0 + kTile);
-    } else {
+        pu = cols[blockIdx.x].right + k;
+        pv = cols[(tx + 1 == tiles_x) ? blockIdx.x - tx : blockIdx.x + 1].left + k;
+    } else {                                                 // bottom row -- top row of the tile below
         k = b - kTile; mask = rec.bottom_row;
-        u = (Y0 + kTile - 1) * L + X0 + k;
-        v = ((Y0 + kTile == L) ? 0u : Y0 + kTile) * L + X0 + k;
+        pu = labels + (uint64_t)(Y0 + kTile - 1) * L + X0 + k;
+        pv = labels + (uint64_t)((Y0 + kTile == L) ? 0u : Y0 + kTile) * L + X0 + k;
     }
     const bool on = (mask >> k) & 1ull;
     uint32_t lu = 0, lv = 0;
-    if (on) { lu = ld_label(labels, u); lv = ld_label(labels, v); }
+    if (on) { lu = __ldcg(pu); lv = __ldcg(pv); }
     // the previous border bond joins the same two tile-local components: nothing new to learn
     const uint32_t plu = __shfl_up_sync(0xFFFFFFFFu, lu, 1), plv = __shfl_up_sync(0xFFFFFFFFu, lv, 1);
     const bool pon = __shfl_up_sync(0xFFFFFFFFu, (uint32_t)on, 1) != 0;
@@ -319,29 +328,56 @@ k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, Params P)
 // it, at a smaller root anywhere.  `rootbits` says which sites are tile-local roots, so each
 // distinct root seen by the tile is chased and drawn ONCE (work spread over the whole CTA) and
 // every other site needs one shared-memory lookup.
+//
+// Memory layout of the accesses: a tile row of labels is 256 bytes = 16 lanes x 16 bytes, so one
+// warp-wide 16-byte access covers two full tile rows (4 wavefronts of 128 contiguous bytes, the
+// minimum).  A CTA of kFlipThreads threads owns a tile; warp w owns kFlipRows = 2 kFlipAcc tile rows;
+// its k-th access covers rows kFlipRows w + 2k and + 2k + 1; lane l holds the 4 sites
+// x = 4 (l % 16) .. + 3 of row kFlipRows w + 2k + l / 16.
+
+#ifndef SW_FLIP_THREADS
+#define SW_FLIP_THREADS 256
+#endif
+#ifndef SW_FLIP_MINB
+#define SW_FLIP_MINB 5
+#endif
+constexpr int kFlipThreads = SW_FLIP_THREADS;
+constexpr int kFlipAcc = (int)kTileSites / (4 * kFlipThreads);   // 16-byte accesses per thread
+constexpr int kFlipRows = 2 * kFlipAcc;                          // tile rows per warp
 
 template <bool kPow2>
-__global__ void __launch_bounds__(kTileThreads)
+__global__ void __launch_bounds__(kFlipThreads, SW_FLIP_MINB)
 k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__restrict__ spins,
             Params P, int write_labels)
 {
     __shared__ uint32_t s_root[kTileSites];                   // per tile-local root: its canonical root
     __shared__ uint8_t s_state[kTileSites];                   // per tile-local root: the new state
-    __shared__ uint16_t s_list[kTileThreads / 32][512];       // per warp: the tile-local roots of its 8 rows
+    __shared__ uint16_t s_list[kFlipThreads / 32][kFlipRows * kTile];   // per warp: the tile-local roots of its rows
 
-    const uint32_t tid = threadIdx.x, y = tid >> 2, c = tid & 3;
+    const uint32_t tid = threadIdx.x;
     const uint32_t lane = tid & 31u, warp = tid >> 5;
     const uint32_t L = P.L, tiles_x = L >> 6;
     const uint32_t ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
     const uint32_t X0 = tx << 6, Y0 = ty << 6;
-    const uint64_t row_off = (uint64_t)(Y0 + y) * L;
-    const uint32_t gx = X0 + (c << 4);
-    const uint32_t i0 = (uint32_t)(row_off + gx);
     const uint32_t origin = Y0 * L + X0;
-    const uint32_t base = (y << 6) + (c << 4);
+    const uint32_t x4 = (lane & 15u) << 2;                     // my first column inside the tile
+    const uint32_t yk0 = warp * kFlipRows + (lane >> 4);       // my tile row for k = 0 (k-th: + 2k)
+    const uint32_t i00 = origin + yk0 * L + x4;                // global index of my first site for k = 0
 
-    // -- phase A: each warp lists the tile-local roots of its strip (prefix sum over the lanes, no atomics)
-    const uint32_t work = rootbits[i0 >> 4];
+    // -- phase A: everything this tile needs from HBM is requested at once: my labels and root flags.
+    //    A tile-local root's own entry is its link into the global forest (itself if the merge never hooked
+    //    it), so the first step of every chase comes out of this coalesced load instead of a scattered one.
+    uint32_t lab[4 * kFlipAcc];
+    uint32_t work = 0;                                         // bit 4k + j: my site j of access k is a tile-local root
+#pragma unroll
+    for (int k = 0; k < kFlipAcc; ++k) {
+        const uint32_t i0 = i00 + 2 * k * L;
+        const uint4 l = __ldcg(reinterpret_cast<const uint4 *>(labels + i0));
+        lab[4 * k] = l.x; lab[4 * k + 1] = l.y; lab[4 * k + 2] = l.z; lab[4 * k + 3] = l.w;
+        const uint32_t rb = rootbits[i0 >> 4];
+        work |= ((rb >> (x4 & 12u)) & 15u) << (4 * k);
+    }
+    // each warp lists the tile-local roots of its strip (prefix sum over the lanes, no atomics)
     uint32_t n_warp;
     {
         const uint32_t n = __popc(work);
@@ -352,10 +388,14 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
             if (lane >= (uint32_t)o) incl += up;
         }
         n_warp = __shfl_sync(0xFFFFFFFFu, incl, 31);
-        uint32_t pos = incl - n, m = work;
-        while (m) {
-            s_list[warp][pos++] = (uint16_t)(base + __ffs(m) - 1);
-            m &= m - 1;
+        uint32_t pos = incl - n;
+#pragma unroll
+        for (int j = 0; j < 4 * kFlipAcc; ++j) {
+            if ((work >> j) & 1u) {
+                const uint32_t id = ((yk0 + 2 * (j >> 2)) << 6) + x4 + (j & 3);
+                s_list[warp][pos++] = (uint16_t)id;
+                s_root[id] = lab[j];                          // where the chase of this root starts
+            }
         }
     }
     __syncwarp();
@@ -364,43 +404,36 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
     for (uint32_t k = lane; k < n_warp; k += 32) {
         const uint32_t id = s_list[warp][k];
         const uint32_t self = origin + (id >> 6) * L + (id & 63u);
-        const uint32_t g = find_root_halving(labels, self);
+        const uint32_t g = find_root_halving_from(labels, self, s_root[id]);
         s_root[id] = g;
         s_state[id] = (uint8_t)flip_state(g, P);
     }
     __syncthreads();
 
     // -- phase C: every site looks its tile-local root up; consecutive sites with the same label share a lookup
-    uint32_t lab[16];
-    {
-        const uint4 *lp = reinterpret_cast<const uint4 *>(labels + row_off + gx);
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const uint4 l = lp[k];
-            lab[4 * k] = l.x; lab[4 * k + 1] = l.y; lab[4 * k + 2] = l.z; lab[4 * k + 3] = l.w;
+    for (int k = 0; k < kFlipAcc; ++k) {
+        const uint32_t i0 = i00 + 2 * k * L;
+        const uint32_t id0 = ((yk0 + 2 * k) << 6) + x4;
+        uint32_t st = 0, prev = 0, root = 0, state = 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const bool isroot = (work >> (4 * k + j)) & 1u;     // a tile-local root stands for itself
+            const uint32_t le = isroot ? i0 + j : lab[4 * k + j];
+            if (j == 0 || le != prev) {
+                const uint32_t d = le - origin;
+                const uint32_t dy = kPow2 ? (d >> P.log2L) : (uint32_t)(((uint64_t)d * P.divL_magic) >> 40);
+                const uint32_t id = isroot ? id0 + j : (dy << 6) + (d - dy * L);
+                root = s_root[id];
+                state = s_state[id];
+                prev = le;
+            }
+            lab[4 * k + j] = root;
+            st |= state << (8 * j);
         }
-    }
-    uint32_t st[4] = {0, 0, 0, 0};
-    uint32_t prev = 0, root = 0, state = 0;
-#pragma unroll
-    for (int j = 0; j < 16; ++j) {
-        const uint32_t le = ((work >> j) & 1u) ? i0 + j : lab[j];   // a tile-local root stands for itself
-        if (j == 0 || le != prev) {
-            const uint32_t d = le - origin;
-            const uint32_t dy = kPow2 ? (d >> P.log2L) : (uint32_t)(((uint64_t)d * P.divL_magic) >> 40);
-            const uint32_t id = (dy << 6) + (d - dy * L);
-            root = s_root[id];
-            state = s_state[id];
-            prev = le;
-        }
-        lab[j] = root;
-        st[j >> 2] |= state << (8 * (j & 3));
-    }
-    *reinterpret_cast<uint4 *>(spins + row_off + gx) = make_uint4(st[0], st[1], st[2], st[3]);
-    if (write_labels) {
-        uint4 *lp = reinterpret_cast<uint4 *>(labels + row_off + gx);
-#pragma unroll
-        for (int k = 0; k < 4; ++k) lp[k] = make_uint4(lab[4 * k], lab[4 * k + 1], lab[4 * k + 2], lab[4 * k + 3]);
+        *reinterpret_cast<uint32_t *>(spins + i0) = st;
+        if (write_labels)
+            *reinterpret_cast<uint4 *>(labels + i0) = make_uint4(lab[4 * k], lab[4 * k + 1], lab[4 * k + 2], lab[4 * k + 3]);
     }
 }
 
