@@ -76,7 +76,7 @@ struct sw_ctx {
     uint32_t *d_sizes = nullptr;          // lazily allocated 4N-byte scratch for cluster sizes
     uint64_t launches = 0, sweeps = 0;
     int num_sms = 148;
-    int tile_variant = 0;                 // development switch (env SW_TILE_VARIANT): 0 = warp per tile, 1 = CTA per tile
+    int tile_variant = 1;                 // development switch (env SW_TILE_VARIANT): 0 = warp per tile, 1 = CTA per tile
     // profiling
     bool profiling = false;
     struct Ev { int slot; cudaEvent_t a, b; };
@@ -161,7 +161,7 @@ int sweep_once(sw_ctx *c)
           else
               sw::k_tile_bonds_label<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_cols, P); }
         { Timed tm(c, SLOT_MERGE);
-          sw::k_tile_merge<<<tiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_cols, P); }
+          sw::k_tile_merge<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_cols, P, tiles); }
         { Timed tm(c, SLOT_FLIP);
           if (P.log2L != 0xFFFFFFFFu)
               sw::k_tile_flip<true><<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->lazy ? 0 : 1);

@@ -290,36 +290,71 @@ k_tile_bonds_label(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bon
 }
 
 // ---- kernel 2: merge across tile borders -------------------------------------------------------
-// One CTA per tile, one thread per border site (64 on the right column, 64 on the bottom row).
+// One thread per border site (64 on the right column, 64 on the bottom row of a tile).  Only about a
+// third of them carry a link worth uniting (active bond, not a repeat of its neighbour's link), and a
+// unite is a chain of dependent L2 / HBM round trips, so the kernel is latency-bound: a CTA therefore
+// gathers the links of kMergeTiles tiles into a dense list first (coalesced loads, all independent)
+// and then unites them with every lane busy.
+
+constexpr int kMergeTiles = 4;
 
 __global__ void __launch_bounds__(kMergeThreads)
-k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, const TileCols *__restrict__ cols, Params P)
+k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, const TileCols *__restrict__ cols,
+             Params P, uint32_t n_tiles)
 {
-    const uint32_t b = threadIdx.x;
+    __shared__ uint2 s_link[kMergeTiles * kMergeThreads];
+    __shared__ uint32_t s_n;
+
+    const uint32_t b = threadIdx.x, lane = b & 31u;
     const uint32_t L = P.L, tiles_x = L >> 6;
-    const uint32_t ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
-    const uint32_t X0 = tx << 6, Y0 = ty << 6;
-    const TileBorder rec = border[blockIdx.x];
-    const uint32_t *pu, *pv;
-    unsigned long long mask;
-    uint32_t k;
-    if (b < kTile) {                                         // right column -- left column of the tile on the right
-        k = b; mask = rec.right_col;
-        pu = cols[blockIdx.x].right + k;
-        pv = cols[(tx + 1 == tiles_x) ? blockIdx.x - tx : blockIdx.x + 1].left + k;
-    } else {                                                 // bottom row -- top row of the tile below
-        k = b - kTile; mask = rec.bottom_row;
-        pu = labels + (uint64_t)(Y0 + kTile - 1) * L + X0 + k;
-        pv = labels + (uint64_t)((Y0 + kTile == L) ? 0u : Y0 + kTile) * L + X0 + k;
+    if (b == 0) s_n = 0;
+    __syncthreads();
+
+    uint32_t lu[kMergeTiles], lv[kMergeTiles];
+    bool on[kMergeTiles];
+#pragma unroll
+    for (int i = 0; i < kMergeTiles; ++i) {
+        const uint32_t tile = blockIdx.x * kMergeTiles + i;
+        on[i] = false; lu[i] = 0; lv[i] = 0;
+        if (tile < n_tiles) {
+            const uint32_t ty = tile / tiles_x, tx = tile - ty * tiles_x;
+            const uint32_t X0 = tx << 6, Y0 = ty << 6;
+            const TileBorder rec = border[tile];
+            const uint32_t *pu, *pv;
+            unsigned long long mask;
+            uint32_t k;
+            if (b < kTile) {                                 // right column -- left column of the tile on the right
+                k = b; mask = rec.right_col;
+                pu = cols[tile].right + k;
+                pv = cols[(tx + 1 == tiles_x) ? tile - tx : tile + 1].left + k;
+            } else {                                         // bottom row -- top row of the tile below
+                k = b - kTile; mask = rec.bottom_row;
+                pu = labels + (uint64_t)(Y0 + kTile - 1) * L + X0 + k;
+                pv = labels + (uint64_t)((Y0 + kTile == L) ? 0u : Y0 + kTile) * L + X0 + k;
+            }
+            on[i] = (mask >> k) & 1ull;
+            if (on[i]) { lu[i] = __ldcg(pu); lv[i] = __ldcg(pv); }
+        }
     }
-    const bool on = (mask >> k) & 1ull;
-    uint32_t lu = 0, lv = 0;
-    if (on) { lu = __ldcg(pu); lv = __ldcg(pv); }
-    // the previous border bond joins the same two tile-local components: nothing new to learn
-    const uint32_t plu = __shfl_up_sync(0xFFFFFFFFu, lu, 1), plv = __shfl_up_sync(0xFFFFFFFFu, lv, 1);
-    const bool pon = __shfl_up_sync(0xFFFFFFFFu, (uint32_t)on, 1) != 0;
-    const bool dup = (b & 31u) != 0 && pon && plu == lu && plv == lv;
-    if (on && !dup) unite(labels, lu, lv);
+#pragma unroll
+    for (int i = 0; i < kMergeTiles; ++i) {
+        // the previous border bond joins the same two tile-local components: nothing new to learn
+        const uint32_t plu = __shfl_up_sync(0xFFFFFFFFu, lu[i], 1), plv = __shfl_up_sync(0xFFFFFFFFu, lv[i], 1);
+        const bool pon = __shfl_up_sync(0xFFFFFFFFu, (uint32_t)on[i], 1) != 0;
+        const bool dup = lane != 0 && pon && plu == lu[i] && plv == lv[i];
+        const bool keep = on[i] && !dup;
+        const uint32_t m = __ballot_sync(0xFFFFFFFFu, keep);
+        uint32_t base = 0;
+        if (lane == 0 && m) base = atomicAdd(&s_n, (uint32_t)__popc(m));
+        base = __shfl_sync(0xFFFFFFFFu, base, 0);
+        if (keep) s_link[base + __popc(m & ((1u << lane) - 1u))] = make_uint2(lu[i], lv[i]);
+    }
+    __syncthreads();
+    const uint32_t n = s_n;
+    for (uint32_t k = b; k < n; k += kMergeThreads) {
+        const uint2 e = s_link[k];
+        unite(labels, e.x, e.y);
+    }
 }
 
 // ---- kernel 3: flatten to the canonical root + flip --------------------------------------------
