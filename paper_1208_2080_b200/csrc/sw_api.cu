@@ -7,7 +7,6 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
-#include <cstdlib>
 #include <new>
 #include <string>
 #include <vector>
@@ -16,7 +15,6 @@
 #include "sw_generic.cuh"
 #include "sw_observe.cuh"
 #include "sw_tiled.cuh"
-#include "sw_tile_warp.cuh"
 
 namespace {
 
@@ -76,7 +74,6 @@ struct sw_ctx {
     uint32_t *d_sizes = nullptr;          // lazily allocated 4N-byte scratch for cluster sizes
     uint64_t launches = 0, sweeps = 0;
     int num_sms = 148;
-    int tile_variant = 1;                 // development switch (env SW_TILE_VARIANT): 0 = warp per tile, 1 = CTA per tile
     // profiling
     bool profiling = false;
     struct Ev { int slot; cudaEvent_t a, b; };
@@ -156,10 +153,7 @@ int sweep_once(sw_ctx *c)
     if (c->tiled) {
         const unsigned tiles = (unsigned)(c->N / sw::kTileSites);
         { Timed tm(c, SLOT_TILE);
-          if (c->tile_variant == 0)
-              sw::k_tile_warp<<<(tiles + sw::kTwWarps - 1) / sw::kTwWarps, sw::kTwThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_cols, P, tiles);
-          else
-              sw::k_tile_bonds_label<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_cols, P); }
+          sw::k_tile_bonds_label<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_cols, P); }
         { Timed tm(c, SLOT_MERGE);
           sw::k_tile_merge<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_cols, P, tiles); }
         { Timed tm(c, SLOT_FLIP);
@@ -250,7 +244,6 @@ int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed,
     cudaError_t e = cudaGetDevice(&c->device);
     if (e != cudaSuccess) { delete c; return SW_ERR_CUDA; }
     cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
-    if (const char *v = getenv("SW_TILE_VARIANT")) c->tile_variant = atoi(v);
     if (external) {
         if (!dev_ws || ws_bytes < plan.total || ((uintptr_t)dev_ws % kAlign) != 0) { delete c; return dev_ws ? SW_ERR_OOM : SW_ERR_INVALID_ARG; }
         c->ws = (uint8_t *)dev_ws; c->stream = (cudaStream_t)stream;
