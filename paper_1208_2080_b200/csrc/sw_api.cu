@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -15,6 +16,7 @@
 #include "sw_generic.cuh"
 #include "sw_observe.cuh"
 #include "sw_tiled.cuh"
+#include "sw_tile_blocks.cuh"
 
 namespace {
 
@@ -58,7 +60,7 @@ struct sw_ctx {
     uint32_t L = 0, q = 0, flags = 0;
     uint64_t N = 0, seed = 0, T = 0, t = 0;
     double K = 0;
-    bool tiled = false, lazy = false;
+    bool tiled = false, lazy = false, tile_runs = false;
     bool have_spins = false, have_labels = false, labels_flat = false;
     bool owns_ws = false, owns_stream = false;
     int device = 0;
@@ -153,7 +155,10 @@ int sweep_once(sw_ctx *c)
     if (c->tiled) {
         const unsigned tiles = (unsigned)(c->N / sw::kTileSites);
         { Timed tm(c, SLOT_TILE);
-          sw::k_tile_bonds_label<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_cols, P); }
+          if (c->tile_runs)
+              sw::k_tile_bonds_label<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_cols, P);
+          else
+              sw::k_tile_blocks<<<tiles, sw::kBlkThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_cols, P); }
         { Timed tm(c, SLOT_MERGE);
           sw::k_tile_merge<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_cols, P, tiles); }
         { Timed tm(c, SLOT_FLIP);
@@ -240,6 +245,7 @@ int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed,
     c->N = (uint64_t)L * L;
     c->tiled = tiled_ok(L, flags);
     c->lazy = (flags & SW_FLAG_LAZY_LABELS) != 0;
+    { const char *e = getenv("SW_TILE_KERNEL"); c->tile_runs = e && !strcmp(e, "runs"); }
     const Plan plan = make_plan(L, q, flags);
     cudaError_t e = cudaGetDevice(&c->device);
     if (e != cudaSuccess) { delete c; return SW_ERR_CUDA; }
