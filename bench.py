@@ -40,8 +40,8 @@ HBM_FALLBACK_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md, used o
 
 # Algorithmic bytes per site per launch.
 BYTES_PER_SITE = {
-    "k_tile_bonds_label": 1.0 + 0.25 + 4.0 + 0.125 + 16.0 / 4096.0,  # spins R, bond bits W, labels W, root bitmap W, border record W
-    "k_tile_merge": 16.0 / 4096.0 + 2 * 4.0 * 2.0 / 64.0 * 0.5,      # border record R + two label reads per ACTIVE border bond (~half)
+    "k_tile_blocks": 1.0 + 0.25 + 4.0 + 0.125 + (16.0 + 1024.0) / 4096.0,  # spins R, bond bits W, labels W, root bitmap W, border + edge records W
+    "k_tile_merge": (16.0 + 1024.0) / 4096.0,                    # border + edge records R (root links touched by the unions come on top)
     "k_tile_flip": 4.0 + 0.125 + 4.0 + 1.0,                          # labels R, root bitmap R, canonical labels W, spins W
 }
 BYTES_PER_SITE_LAZY = dict(BYTES_PER_SITE, k_tile_flip=4.0 + 0.125 + 1.0)

@@ -4,6 +4,7 @@
 // one returns SW_ERR_CUDA.
 #include "../../include/sw.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -25,14 +26,14 @@ using sw::Params;
 enum Slot { SLOT_TILE = 0, SLOT_MERGE = 1, SLOT_FLIP = 2, SLOT_G_BONDS = 3, SLOT_G_INIT = 4,
             SLOT_G_UNION = 5, SLOT_G_FLATTEN = 6, SLOT_G_FLIP = 7 };
 const char *const kSlotNames[SW_MAX_KERNEL_SLOTS] = {
-    "k_tile_bonds_label", "k_tile_merge", "k_tile_flip", "k_bonds_generic", "k_label_identity",
+    "k_tile_blocks", "k_tile_merge", "k_tile_flip", "k_bonds_generic", "k_label_identity",
     "k_union_generic", "k_flatten_generic", "k_flip_generic"};
 
 constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Plan {
-    size_t spins, bonds, labels, rootbits, border, cols, row, flag, total;   // byte offsets into the workspace
+    size_t spins, bonds, labels, rootbits, border, edges, row, flag, total;   // byte offsets into the workspace
 };
 
 bool tiled_ok(uint32_t L, uint32_t flags) { return (L % sw::kTile == 0) && !(flags & SW_FLAG_FORCE_GENERIC); }
@@ -47,7 +48,7 @@ Plan make_plan(uint32_t L, uint32_t q, uint32_t flags)
     p.labels = off; off = align_up(off + N * 4);
     p.rootbits = off; off = align_up(off + (tiled_ok(L, flags) ? (N / 16) * 2 : 0));
     p.border = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileBorder) : 0));
-    p.cols = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileCols) : 0));
+    p.edges = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileEdges) : 0));
     p.row = off;    off = align_up(off + (3 + (size_t)q) * 8);
     p.flag = off;   off = align_up(off + 4);
     p.total = off;
@@ -60,7 +61,7 @@ struct sw_ctx {
     uint32_t L = 0, q = 0, flags = 0;
     uint64_t N = 0, seed = 0, T = 0, t = 0;
     double K = 0;
-    bool tiled = false, lazy = false, tile_runs = false;
+    bool tiled = false, lazy = false;
     bool have_spins = false, have_labels = false, labels_flat = false;
     bool owns_ws = false, owns_stream = false;
     int device = 0;
@@ -71,7 +72,7 @@ struct sw_ctx {
     uint32_t *d_bonds = nullptr, *d_labels = nullptr, *d_flag = nullptr;
     uint16_t *d_rootbits = nullptr;
     sw::TileBorder *d_border = nullptr;
-    sw::TileCols *d_cols = nullptr;
+    sw::TileEdges *d_edges = nullptr;
     unsigned long long *d_row = nullptr;
     uint32_t *d_sizes = nullptr;          // lazily allocated 4N-byte scratch for cluster sizes
     uint64_t launches = 0, sweeps = 0;
@@ -155,17 +156,14 @@ int sweep_once(sw_ctx *c)
     if (c->tiled) {
         const unsigned tiles = (unsigned)(c->N / sw::kTileSites);
         { Timed tm(c, SLOT_TILE);
-          if (c->tile_runs)
-              sw::k_tile_bonds_label<<<tiles, sw::kTileThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_cols, P);
-          else
-              sw::k_tile_blocks<<<tiles, sw::kBlkThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_cols, P); }
+          sw::k_tile_blocks<<<tiles, sw::kBlkThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_edges, P); }
         { Timed tm(c, SLOT_MERGE);
-          sw::k_tile_merge<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_cols, P, tiles); }
+          sw::k_tile_merge<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_edges, P, tiles); }
         { Timed tm(c, SLOT_FLIP);
-          if (P.log2L != 0xFFFFFFFFu)
-              sw::k_tile_flip<true><<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->lazy ? 0 : 1);
+          if (c->lazy)
+              sw::k_tile_flip<false, true><<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P);
           else
-              sw::k_tile_flip<false><<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->lazy ? 0 : 1); }
+              sw::k_tile_flip<true, true><<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P); }
         c->labels_flat = !c->lazy;
     } else {
         const int th = 256;
@@ -194,7 +192,10 @@ int ensure_flat(sw_ctx *c)
     if (c->labels_flat) return SW_OK;
     const Params P = make_params(c, c->t);
     c->launches += 1;
-    sw::k_flatten_generic<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_labels, P);
+    if (c->tiled)       // lazy mode: the forest of the last sweep is still in place (tile-local ids + root links)
+        sw::k_tile_flip<true, false><<<(unsigned)(c->N / sw::kTileSites), sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P);
+    else
+        sw::k_flatten_generic<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_labels, P);
     SW_CUDA(c, cudaGetLastError());
     c->labels_flat = true;
     return SW_OK;
@@ -245,7 +246,6 @@ int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed,
     c->N = (uint64_t)L * L;
     c->tiled = tiled_ok(L, flags);
     c->lazy = (flags & SW_FLAG_LAZY_LABELS) != 0;
-    { const char *e = getenv("SW_TILE_KERNEL"); c->tile_runs = e && !strcmp(e, "runs"); }
     const Plan plan = make_plan(L, q, flags);
     cudaError_t e = cudaGetDevice(&c->device);
     if (e != cudaSuccess) { delete c; return SW_ERR_CUDA; }
@@ -265,7 +265,7 @@ int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed,
     c->d_labels = (uint32_t *)(c->ws + plan.labels);
     c->d_rootbits = (uint16_t *)(c->ws + plan.rootbits);
     c->d_border = (sw::TileBorder *)(c->ws + plan.border);
-    c->d_cols = (sw::TileCols *)(c->ws + plan.cols);
+    c->d_edges = (sw::TileEdges *)(c->ws + plan.edges);
     c->d_row = (unsigned long long *)(c->ws + plan.row);
     c->d_flag = (uint32_t *)(c->ws + plan.flag);
     *out = c;

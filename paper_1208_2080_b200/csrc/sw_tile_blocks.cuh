@@ -112,7 +112,7 @@ __device__ __forceinline__ uint32_t slot_of4(uint32_t W, uint32_t c)
 __global__ void __launch_bounds__(kBlkThreads, 8)
 k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
               uint32_t *__restrict__ labels, uint16_t *__restrict__ rootbits,
-              TileBorder *__restrict__ border, TileCols *__restrict__ cols, Params P)
+              TileBorder *__restrict__ border, TileEdges *__restrict__ edges, Params P)
 {
     __shared__ BlkShared S;
 
@@ -331,7 +331,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
     }
     __syncthreads();                                           // B4: no hooks happen any more
 
-    // -- every component: its root (chase; compress my own entry only), the root's global index, root flag
+    // -- every component: its root (chase; compress my own entry only) and root flag
     uint32_t rootm = ~todo;                                    // a site without any bond is its own cluster
     {
         volatile uint16_t *par = S.parent;
@@ -344,12 +344,14 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
                 par[id] = (uint16_t)r;
             }
             rootm |= (uint32_t)(r == id) << (e >> 16);
-            S.list[k][tid] = origin + (r >> 6) * L + (r & 63u);
+            S.list[k][tid] = r;
         }
     }
 
-    // -- labels: global index of the tile-local root of every site; root bitmap; column labels for the merge
+    // -- labels: a tile-local root keeps its own global index (the merge links it from there), every other site
+    //    gets the tile-local id of its root; root bitmap; roots of the edge sites as global indices for the merge
     const bool five = __any_sync(0xFFFFFFFFu, n > 16u);
+    auto global_of = [&](uint32_t v) { return origin + (v >> 6) * L + (v & 63u); };
     uint32_t col_l[4], col_r[4];
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
@@ -359,14 +361,14 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
         if (!five) {
 #pragma unroll
             for (int c = 0; c < 8; ++c) {
-                const uint32_t g = S.list[slot_of4(Wr, c)][tid];
-                lab[c] = ((todo >> (8 * r + c)) & 1u) ? g : self + c;
+                const uint32_t v = S.list[slot_of4(Wr, c)][tid];
+                lab[c] = ((rootm >> (8 * r + c)) & 1u) ? self + c : v;
             }
         } else {
 #pragma unroll
             for (int c = 0; c < 8; ++c) {
-                const uint32_t g = S.list[slot_of(Wr, Vr, c)][tid];
-                lab[c] = ((todo >> (8 * r + c)) & 1u) ? g : self + c;
+                const uint32_t v = S.list[slot_of(Wr, Vr, c)][tid];
+                lab[c] = ((rootm >> (8 * r + c)) & 1u) ? self + c : v;
             }
         }
         uint4 *lp = reinterpret_cast<uint4 *>(labels + (uint64_t)(y0 + r) * L + x0);
@@ -374,6 +376,14 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
         lp[1] = make_uint4(lab[4], lab[5], lab[6], lab[7]);
         col_l[r] = lab[0];
         col_r[r] = lab[7];
+        if ((r == 0 && by == 0u) || (r == 3 && by == 15u)) {   // top / bottom row of the tile
+            uint32_t g[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) g[c] = ((rootm >> (8 * r + c)) & 1u) ? lab[c] : global_of(lab[c]);
+            uint4 *ep = reinterpret_cast<uint4 *>((r == 0 ? edges[blockIdx.x].top : edges[blockIdx.x].bottom) + 8u * bx);
+            ep[0] = make_uint4(g[0], g[1], g[2], g[3]);
+            ep[1] = make_uint4(g[4], g[5], g[6], g[7]);
+        }
     }
     {
         const uint32_t pm = __shfl_xor_sync(0xFFFFFFFFu, rootm, 1);
@@ -384,8 +394,16 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
             rootbits[(i0 + r * L) >> 4] = (uint16_t)(((me >> (8 * r)) & 0xFFu) | (((mo >> (8 * r)) & 0xFFu) << 8));
         }
     }
-    if (bx == 0u) *reinterpret_cast<uint4 *>(cols[blockIdx.x].left + 4u * by) = make_uint4(col_l[0], col_l[1], col_l[2], col_l[3]);
-    if (bx == 7u) *reinterpret_cast<uint4 *>(cols[blockIdx.x].right + 4u * by) = make_uint4(col_r[0], col_r[1], col_r[2], col_r[3]);
+    if (bx == 0u || bx == 7u) {                               // left / right column of the tile
+        const uint32_t c = bx == 0u ? 0u : 7u;
+        uint32_t g[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const uint32_t v = bx == 0u ? col_l[r] : col_r[r];
+            g[r] = ((rootm >> (8 * r + c)) & 1u) ? v : global_of(v);
+        }
+        *reinterpret_cast<uint4 *>((bx == 0u ? edges[blockIdx.x].left : edges[blockIdx.x].right) + 4u * by) = make_uint4(g[0], g[1], g[2], g[3]);
+    }
 }
 
 }  // namespace sw

@@ -214,5 +214,5 @@ def test_profile_slots():
     g.profile_begin()
     g.sweep(5)
     prof = g.profile_end()
-    assert set(prof) == {"k_tile_bonds_label", "k_tile_merge", "k_tile_flip"}
+    assert set(prof) == {"k_tile_blocks", "k_tile_merge", "k_tile_flip"}
     assert all(v["launches"] == 5 and v["ms"] > 0 for v in prof.values())
