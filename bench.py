@@ -46,6 +46,12 @@ BYTES_PER_SITE = {
 }
 BYTES_PER_SITE_LAZY = dict(BYTES_PER_SITE, k_tile_flip=4.0 + 0.125 + 1.0)
 
+# The tile kernel is bound by instruction issue, not by HBM (profiles/README.md), so it is ALSO reported against an
+# integer-ALU roofline: algorithmic lane-operations per site = 0.5 Philox4x32-10 calls x (20 32x32->64
+# multiplies + 20 three-input XORs) + 2 threshold compares + 2 spin compares; peak = SMs x 128 lanes x SM clock.
+ALU_OPS_PER_SITE = {"k_tile_blocks": 0.5 * 40 + 2 + 2}
+B200_SMS, B200_LANES_PER_SM = 148, 128
+
 
 def rank_info():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
@@ -276,6 +282,15 @@ def run_gpu(args):
                     "frac": (a / peak) if a else None, "traffic": ncu_traffic(args.workload, top),
                     "peak_source": peak_src,
                     "algorithmic_bytes_per_launch": bps.get(top, 0) * N}
+    roofline_alu = None
+    if kernels and roofline and roofline["kernel"] in ALU_OPS_PER_SITE:
+        clk = ((clocks or {}).get("sm_mhz") or 1965.0) * 1e6
+        ops = ALU_OPS_PER_SITE[roofline["kernel"]] * N
+        a = ops / (kernels[roofline["kernel"]]["ms_per_launch"] * 1e-3) / 1e12
+        pk = B200_SMS * B200_LANES_PER_SM * clk / 1e12
+        roofline_alu = {"kernel": roofline["kernel"], "bound": "alu", "achieved": a, "peak": pk, "unit": "Tlane-op/s",
+                        "frac": a / pk, "algorithmic_ops_per_launch": ops,
+                        "peak_source": "148 SMs x 128 int32 lanes x SM clock under load (B200_PROFILING.md unit counts)"}
     sweep_bytes = sum(v for v in bps.values()) * N
     sweep_floor_ms = sweep_bytes / (peak * 1e9) * 1e3
     per_gpu_ms = elapsed_ms / args.steps
@@ -305,6 +320,7 @@ def run_gpu(args):
                 "what": "sw_set_state(host spins) + sw_sweep(1) + sw_get_spins(host) per step, pinned host memory"},
         "gpu_launches": launches,
         "roofline": roofline,
+        "roofline_alu": roofline_alu,
         "cpu_baseline": cpu_baseline,
         "kernels": kernels,
         "sweep_model": {"bytes_per_site": sum(bps.values()), "floor_ms_at_peak": sweep_floor_ms,
