@@ -118,6 +118,20 @@ def spins_blocks(L: int, q: int, block: int, seed: int) -> np.ndarray:
     return np.ascontiguousarray(np.kron(coarse, np.ones((block, block), dtype=np.uint8))[:L, :L])
 
 
+def spins_dominoes(L: int, dx: int, dy: int, vertical: bool, q: int = 251) -> np.ndarray:
+    """A tiling by 1 x 2 (or 2 x 1) dominoes shifted by (dx, dy), each domino with its own state (distinct from its
+    neighbours' except for rare hash collisions): with K = inf every domino is one cluster, the densest packing of
+    small components a block of the lattice can hold; shifted tilings put half of every border domino in the next
+    block / tile, i.e. as many single-site components with a link out of the block as possible."""
+    y, x = np.mgrid[0:L, 0:L]
+    if vertical:
+        a, b = x, ((y - dy) % L) // 2
+    else:
+        a, b = ((x - dx) % L) // 2, y
+    h = (a.astype(np.uint64) * 0x9E3779B1 + b.astype(np.uint64) * 0x85EBCA77 + 12345) % 0xFFFFFFFB
+    return (h % q).astype(np.uint8)
+
+
 def bonds_random(L: int, density: float, seed: int) -> np.ndarray:
     """Random bond mask, bit0 = right bond of the site, bit1 = its down bond (for labeling tests)."""
     rng = np.random.default_rng(seed)

@@ -126,6 +126,28 @@ def test_adversarial_lattices_generic(L):
         compare_after_sweep(gpu, cpu, f"({name}, L={L})")
 
 
+@pytest.mark.parametrize("vertical", [False, True])
+@pytest.mark.parametrize("shift", [0, 1])
+def test_domino_tilings_fill_every_component_slot(vertical, shift):
+    # 16 two-site components per 8 x 4 block (shift 0) or, shifted, single-site components with a link into the next
+    # block along every block edge: exercises the unbuffered-link path and the five-plane label decode of k_tile_blocks
+    L = 128
+    spins = wl.spins_dominoes(L, shift, shift, vertical)
+    gpu = SwendsenWang(L, 251, math.inf, 3)
+    cpu = Oracle(L, 251, math.inf, 3)
+    gpu.set_state(spins, 2); cpu.set_state(spins, 2)
+    gpu.sweep(1); cpu.sweep(1)
+    compare_after_sweep(gpu, cpu, f"(dominoes vertical={vertical} shift={shift})")
+    assert cpu.measure()["n_clusters"] >= L * L // 2 - 64     # (hash collisions may merge a few dominoes)
+
+
+def test_mixed_small_components_high_q():
+    # q = 5 random spins at K = inf: mostly single sites, pairs and triples; many components per block
+    L = 192
+    spins = wl.spins_uniform_random(L, 5, 3)
+    run_pair(L, 5, math.inf, seed=9, start=None, sweeps=2, spins=spins, t0=1)
+
+
 def test_long_snake_through_every_tile():
     # the spiral path at L = 512 crosses tile borders ~ 4000 times and has diameter ~ 130 000
     L = 512
