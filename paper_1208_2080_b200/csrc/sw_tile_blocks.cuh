@@ -159,24 +159,30 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
 
     // -- step (1): a bond is active iff the spins are equal and its draw is below the threshold
     uint32_t R = 0, D = 0;
+    {
+        // (a rolled loop over the four rows with the rows rotating through registers: the unrolled body is four times
+        //  the code, and with 32 warps in different phases of this kernel the instruction cache is what runs out)
+        uint2 cur = s[0], n1r = s[1], n2r = s[2], n3r = s[3], n4r = s[4];
+#pragma unroll 1
+        for (int r = 0; r < 4; ++r) {
+            const uint32_t a0 = cur.x, a1 = cur.y;
+            const uint32_t n0 = __funnelshift_r(a0, a1, 8), n1 = __funnelshift_r(a1, nx >> (8 * r), 8);
+            const uint32_t eq_r = pack4(__vcmpeq4(a0, n0)) | (pack4(__vcmpeq4(a1, n1)) << 4);
+            const uint32_t eq_d = pack4(__vcmpeq4(a0, n1r.x)) | (pack4(__vcmpeq4(a1, n1r.y)) << 4);
+            const uint32_t pair0 = (i0 + r * L) >> 1;
+            uint32_t m_r = 0, m_d = 0;
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
-        const uint32_t a0 = s[r].x, a1 = s[r].y;
-        const uint32_t n0 = __funnelshift_r(a0, a1, 8), n1 = __funnelshift_r(a1, nx >> (8 * r), 8);
-        const uint32_t eq_r = pack4(__vcmpeq4(a0, n0)) | (pack4(__vcmpeq4(a1, n1)) << 4);
-        const uint32_t eq_d = pack4(__vcmpeq4(a0, s[r + 1].x)) | (pack4(__vcmpeq4(a1, s[r + 1].y)) << 4);
-        const uint32_t pair0 = (i0 + r * L) >> 1;
-        uint32_t m_r = 0, m_d = 0;
-#pragma unroll
-        for (int p = 0; p < 4; ++p) {                          // one Philox call per site pair: right, down, right, down
-            const uint4 d = philox4x32_10(pair0 + p, 0u, P.t, kPurposeBond, P);
-            m_r |= (uint32_t)(d.x <= P.thr_m1) << (2 * p);
-            m_d |= (uint32_t)(d.y <= P.thr_m1) << (2 * p);
-            m_r |= (uint32_t)(d.z <= P.thr_m1) << (2 * p + 1);
-            m_d |= (uint32_t)(d.w <= P.thr_m1) << (2 * p + 1);
+            for (int p = 0; p < 4; ++p) {                      // one Philox call per site pair: right, down, right, down
+                const uint4 d = philox4x32_10(pair0 + p, 0u, P.t, kPurposeBond, P);
+                m_r |= (uint32_t)(d.x <= P.thr_m1) << (2 * p);
+                m_d |= (uint32_t)(d.y <= P.thr_m1) << (2 * p);
+                m_r |= (uint32_t)(d.z <= P.thr_m1) << (2 * p + 1);
+                m_d |= (uint32_t)(d.w <= P.thr_m1) << (2 * p + 1);
+            }
+            R |= (eq_r & m_r) << (8 * r);
+            D |= (eq_d & m_d) << (8 * r);
+            cur = n1r; n1r = n2r; n2r = n3r; n3r = n4r;
         }
-        R |= (eq_r & m_r) << (8 * r);
-        D |= (eq_d & m_d) << (8 * r);
     }
     R &= P.thr_any;
     D &= P.thr_any;
