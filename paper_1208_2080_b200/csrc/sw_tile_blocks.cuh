@@ -64,6 +64,13 @@ __device__ __forceinline__ uint32_t atomic_min_u16(uint16_t *base, uint32_t idx,
 __device__ __forceinline__ void unite_s16(uint16_t *parent_, uint32_t a, uint32_t b)
 {
     volatile uint16_t *parent = parent_;
+    {   // two unconditional hops on both sides first (a root points at itself): most chases end here, branch-free
+        const uint32_t a1 = parent[a], b1 = parent[b];
+        const uint32_t a2 = parent[a1], b2 = parent[b1];
+        if (a2 != a1) parent[a] = (uint16_t)a2;
+        if (b2 != b1) parent[b] = (uint16_t)b2;
+        a = a2; b = b2;
+    }
     while (true) {
         uint32_t pa = parent[a], pb = parent[b];
         while (pa != a || pb != b) {
@@ -343,12 +350,11 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
         volatile uint16_t *par = S.parent;
         for (uint32_t k = 0; k < n; ++k) {
             const uint32_t e = S.list[k][tid], id = e & 0xFFFFu;
-            uint32_t r = par[id];
-            if (r != id) {
-                uint32_t g = par[r];
-                while (g != r) { r = g; g = par[r]; }
-                par[id] = (uint16_t)r;
-            }
+            // three unconditional hops (a root points at itself, so hopping on is harmless), then the rare long chain
+            const uint32_t r1 = par[id], r2 = par[r1];
+            uint32_t r = r2, g = par[r2];
+            while (g != r) { r = g; g = par[r]; }
+            if (r != r1) par[id] = (uint16_t)r;
             rootm |= (uint32_t)(r == id) << (e >> 16);
             S.list[k][tid] = r;
         }
