@@ -33,7 +33,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Plan {
-    size_t spins, bonds, labels, rootbits, border, edges, row, flag, total;   // byte offsets into the workspace
+    size_t spins, bonds, labels, rootbits, border, edges, tile_clusters, row, flag, total;   // byte offsets into the workspace
 };
 
 bool tiled_ok(uint32_t L, uint32_t flags) { return (L % sw::kTile == 0) && !(flags & SW_FLAG_FORCE_GENERIC); }
@@ -49,6 +49,7 @@ Plan make_plan(uint32_t L, uint32_t q, uint32_t flags)
     p.rootbits = off; off = align_up(off + (tiled_ok(L, flags) ? (N / 16) * 2 : 0));
     p.border = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileBorder) : 0));
     p.edges = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileEdges) : 0));
+    p.tile_clusters = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * (sw::kFlipThreads / 32) * 4 : 0));
     p.row = off;    off = align_up(off + (3 + (size_t)q) * 8);
     p.flag = off;   off = align_up(off + 4);
     p.total = off;
@@ -69,7 +70,7 @@ struct sw_ctx {
     uint8_t *ws = nullptr;
     size_t ws_bytes = 0;
     uint8_t *d_spins = nullptr;
-    uint32_t *d_bonds = nullptr, *d_labels = nullptr, *d_flag = nullptr;
+    uint32_t *d_bonds = nullptr, *d_labels = nullptr, *d_flag = nullptr, *d_tile_clusters = nullptr;
     uint16_t *d_rootbits = nullptr;
     sw::TileBorder *d_border = nullptr;
     sw::TileEdges *d_edges = nullptr;
@@ -150,7 +151,8 @@ struct Timed {
     }
 };
 
-int sweep_once(sw_ctx *c)
+// count_clusters: the flip kernel also counts the canonical roots (wanted for the last sweep before a measurement)
+int sweep_once(sw_ctx *c, bool count_clusters)
 {
     const Params P = make_params(c, c->t);
     if (c->tiled) {
@@ -160,10 +162,9 @@ int sweep_once(sw_ctx *c)
         { Timed tm(c, SLOT_MERGE);
           sw::k_tile_merge<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_edges, P, tiles); }
         { Timed tm(c, SLOT_FLIP);
-          if (c->lazy)
-              sw::k_tile_flip<false, true><<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P);
-          else
-              sw::k_tile_flip<true, true><<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P); }
+          auto flip = c->lazy ? (count_clusters ? sw::k_tile_flip<false, true, true> : sw::k_tile_flip<false, true, false>)
+                              : (count_clusters ? sw::k_tile_flip<true, true, true> : sw::k_tile_flip<true, true, false>);
+          flip<<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters); }
         c->labels_flat = !c->lazy;
     } else {
         const int th = 256;
@@ -193,7 +194,7 @@ int ensure_flat(sw_ctx *c)
     const Params P = make_params(c, c->t);
     c->launches += 1;
     if (c->tiled)       // lazy mode: the forest of the last sweep is still in place (tile-local ids + root links)
-        sw::k_tile_flip<true, false><<<(unsigned)(c->N / sw::kTileSites), sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P);
+        sw::k_tile_flip<true, false, false><<<(unsigned)(c->N / sw::kTileSites), sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters);
     else
         sw::k_flatten_generic<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_labels, P);
     SW_CUDA(c, cudaGetLastError());
@@ -208,6 +209,12 @@ int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m
     SW_CUDA(c, cudaMemsetAsync(row, 0, (3 + (size_t)c->q) * 8, c->stream));
     const bool cl = c->have_labels;
     uint32_t want = (want_e ? 1u : 0u) | (want_m ? 2u : 0u) | ((cl && (want_nc || want_big)) ? 4u : 0u);
+    if ((want & 4u) && c->tiled) {      // the flip kernel of the last sweep left one count per tile: no pass over labels[]
+        want &= ~4u;
+        c->launches += 1;
+        const unsigned tiles = (unsigned)(c->N / sw::kTileSites) * (sw::kFlipThreads / 32);   // one count per warp of the flip kernel
+        sw::k_sum_tile_clusters<<<grid_for(c, tiles, sw::kObsThreads), sw::kObsThreads, 0, c->stream>>>(c->d_tile_clusters, tiles, row);
+    }
     if (want) {
         c->launches += 1;
         if (c->L % 16 == 0)
@@ -216,6 +223,10 @@ int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m
             sw::k_observe_scalar<<<grid_for(c, c->N, sw::kObsThreads), sw::kObsThreads, 0, c->stream>>>(c->d_spins, c->d_labels, P, want, row);
     }
     if (cl && want_big) {
+        if (c->tiled) {          // cluster sizes need root pointers: on the tiled path labels[] holds tile-local ids until flattened
+            const int rc = ensure_flat(c);
+            if (rc != SW_OK) return rc;
+        }
         if (!c->d_sizes) SW_CUDA(c, cudaMalloc(&c->d_sizes, c->N * 4));
         SW_CUDA(c, cudaMemsetAsync(c->d_sizes, 0, c->N * 4, c->stream));
         c->launches += 2;
@@ -266,6 +277,7 @@ int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed,
     c->d_rootbits = (uint16_t *)(c->ws + plan.rootbits);
     c->d_border = (sw::TileBorder *)(c->ws + plan.border);
     c->d_edges = (sw::TileEdges *)(c->ws + plan.edges);
+    c->d_tile_clusters = (uint32_t *)(c->ws + plan.tile_clusters);
     c->d_row = (unsigned long long *)(c->ws + plan.row);
     c->d_flag = (uint32_t *)(c->ws + plan.flag);
     *out = c;
@@ -349,7 +361,7 @@ int sw_sweep(sw_ctx *c, uint64_t n)
     if (!c->have_spins) return fail(c, SW_ERR_STATE, "sw_sweep: no spins (call sw_init or sw_set_state)");
     if (c->t + n > 0x100000000ull) return fail(c, SW_ERR_STATE, "sw_sweep: sweep counter would pass 2^32");
     for (uint64_t k = 0; k < n; ++k) {
-        const int rc = sweep_once(c);
+        const int rc = sweep_once(c, k + 1 == n);
         if (rc != SW_OK) return rc;
     }
     SW_CUDA(c, cudaGetLastError());
@@ -388,7 +400,7 @@ int sw_sweep_measure(sw_ctx *c, uint64_t n, uint64_t *out)
     for (uint64_t done = 0; done < n && rc == SW_OK;) {
         const uint64_t m = (n - done < chunk_max) ? n - done : chunk_max;
         for (uint64_t k = 0; k < m && rc == SW_OK; ++k) {
-            rc = sweep_once(c);
+            rc = sweep_once(c, true);
             if (rc == SW_OK) rc = enqueue_observe(c, d_rows + k * stride, true, true, true, true);
         }
         if (rc == SW_OK) {

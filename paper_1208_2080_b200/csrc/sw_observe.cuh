@@ -29,6 +29,16 @@ __device__ __forceinline__ void block_add_u64(unsigned long long v, unsigned lon
     }
 }
 
+// n_clusters on the tiled path: the flip kernel has counted the canonical roots of every tile
+__global__ void __launch_bounds__(kObsThreads)
+k_sum_tile_clusters(const uint32_t *__restrict__ tile_clusters, uint32_t n_tiles, unsigned long long *row)
+{
+    __shared__ unsigned long long s_scratch[kObsThreads / 32];
+    unsigned long long v = 0;
+    for (uint32_t k = blockIdx.x * blockDim.x + threadIdx.x; k < n_tiles; k += gridDim.x * blockDim.x) v += tile_clusters[k];
+    block_add_u64(v, row + 1, s_scratch);
+}
+
 // Scalar version: any L.  want: bit0 energy, bit1 magnetisation, bit2 n_clusters.
 __global__ void __launch_bounds__(kObsThreads)
 k_observe_scalar(const uint8_t *__restrict__ spins, const uint32_t *__restrict__ labels, Params P,

@@ -125,10 +125,12 @@ constexpr int kFlipAcc = (int)kTileSites / (4 * kFlipThreads);   // 16-byte acce
 constexpr int kFlipRows = 2 * kFlipAcc;                          // tile rows per warp
 
 // kLabels: write the canonical labels back (eager mode, or the on-demand flatten of lazy mode);
-// kSpins: draw and write the new spins.
-template <bool kLabels, bool kSpins>
+// kSpins: draw and write the new spins; kCount: leave the number of canonical roots per warp in tile_clusters[]
+// (n_clusters of sw_measure without a pass over labels[]; costs 3 % of the kernel, so only the last sweep of a call does it).
+template <bool kLabels, bool kSpins, bool kCount>
 __global__ void __launch_bounds__(kFlipThreads, 5)
-k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__restrict__ spins, Params P)
+k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__restrict__ spins, Params P,
+            uint32_t *__restrict__ tile_clusters)
 {
     __shared__ uint32_t s_root[kTileSites];                   // per tile-local root: its canonical root
     __shared__ uint8_t s_state[kTileSites];                   // per tile-local root: the new state
@@ -190,6 +192,7 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
     __syncthreads();
 
     // -- phase C: every site looks up (canonical root, new state) of its tile-local root
+    uint32_t canon = 0;                                        // clusters whose smallest site is one of mine (for sw_measure)
 #pragma unroll
     for (int k = 0; k < kFlipAcc; ++k) {
         const uint32_t i0 = i00 + 2 * k * L;
@@ -200,11 +203,16 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
             const bool isroot = (work >> (4 * k + j)) & 1u;     // a tile-local root stands for itself
             const uint32_t id = isroot ? id0 + j : lab[4 * k + j];
             lab[4 * k + j] = s_root[id];
+            if (kCount) canon += (lab[4 * k + j] == i0 + j);    // a canonical root is its own label
             if (kSpins) st |= (uint32_t)s_state[id] << (8 * j);
         }
         if (kSpins) *reinterpret_cast<uint32_t *>(spins + i0) = st;
         if (kLabels)
             *reinterpret_cast<uint4 *>(labels + i0) = make_uint4(lab[4 * k], lab[4 * k + 1], lab[4 * k + 2], lab[4 * k + 3]);
+    }
+    if (kCount) {
+        canon = __reduce_add_sync(0xFFFFFFFFu, canon);
+        if (lane == 0) tile_clusters[blockIdx.x * (kFlipThreads / 32) + warp] = canon;
     }
 }
 

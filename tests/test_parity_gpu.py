@@ -81,6 +81,17 @@ def test_flag_variants_give_identical_results(flags):
     run_pair(192, 2, wl.k_critical(2), seed=5, start="ordered", sweeps=3, flags=flags)
 
 
+def test_lazy_labels_measure_before_any_label_readback():
+    # lazy mode keeps tile-local ids in labels[] until someone asks: cluster statistics must not depend on that
+    g = SwendsenWang(192, 3, wl.k_critical(3), 4, flags=sw.FLAG_LAZY_LABELS)
+    o = Oracle(192, 3, wl.k_critical(3), 4)
+    g.init("random"); o.init("random")
+    for _ in range(3):
+        g.sweep(1); o.sweep(1)
+        assert g.measure() == o.measure()
+    assert np.array_equal(g.get_labels(), o.get_labels())
+
+
 def test_tiled_path_is_selected_and_counts_kernels():
     g = SwendsenWang(128, 2, 0.5, 1)
     g.init("ordered")
