@@ -218,7 +218,7 @@ int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m
     if (want) {
         c->launches += 1;
         if (c->L % 16 == 0)
-            sw::k_observe_vec16<<<grid_for(c, c->N / 16, sw::kObsThreads), sw::kObsThreads, 0, c->stream>>>(c->d_spins, c->d_labels, P, want, row);
+            sw::k_observe_vec16<<<grid_for(c, c->N / 64, sw::kObsThreads), sw::kObsThreads, 0, c->stream>>>(c->d_spins, c->d_labels, P, want, row);
         else
             sw::k_observe_scalar<<<grid_for(c, c->N, sw::kObsThreads), sw::kObsThreads, 0, c->stream>>>(c->d_spins, c->d_labels, P, want, row);
     }

@@ -69,7 +69,7 @@ k_observe_scalar(const uint8_t *__restrict__ spins, const uint32_t *__restrict__
     if (want & 4u) block_add_u64(roots, row + 1, s_scratch);
 }
 
-// Vector version: L % 16 == 0; one thread per 16 consecutive sites of a row.
+// Vector version: L % 16 == 0; one thread per block of 4 rows x 16 consecutive sites.
 __global__ void __launch_bounds__(kObsThreads)
 k_observe_vec16(const uint8_t *__restrict__ spins, const uint32_t *__restrict__ labels, Params P,
                 uint32_t want, unsigned long long *row)
@@ -78,53 +78,68 @@ k_observe_vec16(const uint8_t *__restrict__ spins, const uint32_t *__restrict__ 
     __shared__ unsigned long long s_scratch[kObsThreads / 32];
     for (int k = threadIdx.x; k < 256; k += blockDim.x) s_hist[k] = 0;
     __syncthreads();
-    const uint64_t n_groups = P.N >> 4;
-    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
-    const uint32_t L = P.L, gpr = L >> 4;                  // groups per row
+    // unit of work: 4 rows x 16 columns (L % 16 == 0), so the row below is re-read once per 4 rows, not once per row
+    const uint32_t n_units = (uint32_t)(P.N >> 6);         // <= 2^26: 32-bit index arithmetic throughout
+    const uint32_t stride = gridDim.x * blockDim.x;
+    const uint32_t L = P.L, gpr = L >> 4;                  // 16-site groups per row
     unsigned long long e = 0, roots = 0;
     unsigned int cnt[4] = {0, 0, 0, 0};                    // q <= 4 fast path
-    for (uint64_t g = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; g < n_groups; g += stride) {
-        const uint32_t y = (uint32_t)(g / gpr), gx = (uint32_t)(g - (uint64_t)y * gpr);
-        const uint64_t base = (uint64_t)y * L + ((uint64_t)gx << 4);
-        const uint4 s = *reinterpret_cast<const uint4 *>(spins + base);
-        const uint32_t w[4] = {s.x, s.y, s.z, s.w};
-        if (want & 1u) {
-            const uint32_t next = spins[(uint64_t)y * L + ((gx + 1 == gpr) ? 0u : ((gx + 1) << 4))];
-            const uint32_t yd = (y + 1 == L) ? 0u : y + 1;
-            const uint4 d = *reinterpret_cast<const uint4 *>(spins + (uint64_t)yd * L + ((uint64_t)gx << 4));
-            const uint32_t dw[4] = {d.x, d.y, d.z, d.w};
+    for (uint32_t u = blockIdx.x * blockDim.x + threadIdx.x; u < n_units; u += stride) {
+        const uint32_t y4 = u / gpr, gx = u - y4 * gpr, y0 = y4 << 2;
+        const uint32_t x0 = gx << 4, xn = (gx + 1 == gpr) ? 0u : ((gx + 1) << 4);
+        uint4 rows[5];
+        uint32_t nxt[4];
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const uint32_t hi = (k < 3) ? w[k + 1] : next;
-                const uint32_t r = __funnelshift_r(w[k], hi, 8);             // the right neighbours of the 4 bytes
-                e += (__popc(__vcmpeq4(w[k], r)) + __popc(__vcmpeq4(w[k], dw[k]))) >> 3;
-            }
+        for (int r = 0; r < 4; ++r) {
+            rows[r] = *reinterpret_cast<const uint4 *>(spins + (uint64_t)(y0 + r) * L + x0);
+            if (want & 1u) nxt[r] = spins[(uint64_t)(y0 + r) * L + xn];
         }
-        if (want & 2u) {
-            if (P.q <= 4) {
+        if (want & 1u) rows[4] = *reinterpret_cast<const uint4 *>(spins + (uint64_t)((y0 + 4 == L) ? 0u : y0 + 4) * L + x0);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const uint32_t w[4] = {rows[r].x, rows[r].y, rows[r].z, rows[r].w};
+            if (want & 1u) {
+                const uint32_t dw[4] = {rows[r + 1].x, rows[r + 1].y, rows[r + 1].z, rows[r + 1].w};
+                uint32_t acc = 0;                              // per byte lane: equal pairs seen (<= 8)
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
-#pragma unroll
-                    for (uint32_t a = 0; a < 4; ++a)
-                        cnt[a] += __popc(__vcmpeq4(w[k], a * 0x01010101u)) >> 3;
+                    const uint32_t hi = (k < 3) ? w[k + 1] : nxt[r];
+                    const uint32_t rn = __funnelshift_r(w[k], hi, 8);        // the right neighbours of the 4 bytes
+                    acc += (__vcmpeq4(w[k], rn) & 0x01010101u) + (__vcmpeq4(w[k], dw[k]) & 0x01010101u);
                 }
-            } else {
+                e += (acc * 0x01010101u) >> 24;
+            }
+            if (want & 2u) {
+                if (P.q <= 4) {
+                    // states are two bits per byte: per byte lane, count bit 0, bit 1 and both (each <= 4 over the 4 words)
+                    uint32_t s0 = 0, s1 = 0, s3 = 0;
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    atomicAdd(&s_hist[w[k] & 0xFF], 1u);
-                    atomicAdd(&s_hist[(w[k] >> 8) & 0xFF], 1u);
-                    atomicAdd(&s_hist[(w[k] >> 16) & 0xFF], 1u);
-                    atomicAdd(&s_hist[w[k] >> 24], 1u);
+                    for (int k = 0; k < 4; ++k) {
+                        const uint32_t b0 = w[k] & 0x01010101u, b1 = (w[k] >> 1) & 0x01010101u;
+                        s0 += b0; s1 += b1; s3 += b0 & b1;
+                    }
+                    const uint32_t n3 = (s3 * 0x01010101u) >> 24;
+                    const uint32_t n1 = ((s0 * 0x01010101u) >> 24) - n3, n2 = ((s1 * 0x01010101u) >> 24) - n3;
+                    cnt[0] += 16u - n1 - n2 - n3; cnt[1] += n1; cnt[2] += n2; cnt[3] += n3;
+                } else {
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        atomicAdd(&s_hist[w[k] & 0xFF], 1u);
+                        atomicAdd(&s_hist[(w[k] >> 8) & 0xFF], 1u);
+                        atomicAdd(&s_hist[(w[k] >> 16) & 0xFF], 1u);
+                        atomicAdd(&s_hist[w[k] >> 24], 1u);
+                    }
                 }
             }
-        }
-        if (want & 4u) {
-            const uint4 *lp = reinterpret_cast<const uint4 *>(labels + base);
-            const uint32_t i0 = (uint32_t)base;
+            if (want & 4u) {
+                const uint64_t base = (uint64_t)(y0 + r) * L + x0;
+                const uint4 *lp = reinterpret_cast<const uint4 *>(labels + base);
+                const uint32_t i0 = (uint32_t)base;
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const uint4 l = lp[k];
-                roots += (l.x == i0 + 4 * k) + (l.y == i0 + 4 * k + 1) + (l.z == i0 + 4 * k + 2) + (l.w == i0 + 4 * k + 3);
+                for (int k = 0; k < 4; ++k) {
+                    const uint4 l = lp[k];
+                    roots += (l.x == i0 + 4 * k) + (l.y == i0 + 4 * k + 1) + (l.z == i0 + 4 * k + 2) + (l.w == i0 + 4 * k + 3);
+                }
             }
         }
     }
