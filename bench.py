@@ -172,7 +172,7 @@ def run_gpu(args):
     import torch.distributed as dist
 
     from paper_1208_2080_b200 import replicas
-    from paper_1208_2080_b200.binding import FLAG_DEFAULT, FLAG_LAZY_LABELS, SwendsenWang
+    from paper_1208_2080_b200.binding import FLAG_DEFAULT, FLAG_LABEL_EQUIVALENCE, FLAG_LAZY_LABELS, SwendsenWang
 
     rank, local_rank, world = rank_info()
     if not torch.cuda.is_available():
@@ -186,6 +186,8 @@ def run_gpu(args):
     L, q, K = c["L"], c["q"], c["K"]
     N = L * L
     flags = FLAG_LAZY_LABELS if args.lazy else FLAG_DEFAULT
+    if args.label_equivalence:
+        flags = FLAG_LABEL_EQUIVALENCE
     sim = SwendsenWang(L, q, K, replicas.replica_seed(c["seed"], rank), flags=flags)
     sim.init(c["start"])
     sim.sweep(args.warmup)
@@ -311,7 +313,7 @@ def run_gpu(args):
         "vs_baseline": (value / PAPER_FLIPS_PER_NS) if args.workload == wl.HEADLINE else None,
         "dtype": "u32", "data": "synthetic",
         "config": {"workload": args.workload, "L": L, "q": q, "K": K, "start": c["start"], "seed": c["seed"],
-                   "labels": "lazy" if args.lazy else "canonical every sweep",
+                   "labels": "label equivalence (comparison variant)" if args.label_equivalence else "lazy" if args.lazy else "canonical every sweep",
                    "parallelism": "replicas only" if world > 1 else "1 GPU",
                    "l2": f"working set {stats['device_bytes'] / 2**30:.1f} GiB >> 126 MB L2, no flush needed" if stats["device_bytes"] > (1 << 30)
                          else "working set fits L2: HBM roofline fractions are not meaningful at this size"},
@@ -328,6 +330,7 @@ def run_gpu(args):
         "update_plus_measurement": {"value": value_meas, "unit": UNIT, "steps": m_steps,
                                     "what": "sw_sweep(1) + sw_measure(energy, magnetisation, n_clusters) per step"},
         "last_observables": obs,
+        "label_equivalence_rounds_per_sweep": (stats["le_rounds_total"] / stats["sweeps"]) if args.label_equivalence else None,
         "paper_context": {"flips_per_ns_256xM2050_L65536": PAPER_FLIPS_PER_NS, "flips_per_ns_1xM2050_L4096": 0.232,
                           "source": "PAPER.md:97-103 (Table 1)"},
     }
@@ -345,6 +348,8 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--workload", choices=sorted(wl.CONFIGS), default=wl.HEADLINE)
     ap.add_argument("--lazy", action="store_true", help="SW_FLAG_LAZY_LABELS: canonical labels flattened on demand only")
+    ap.add_argument("--label-equivalence", action="store_true",
+                    help="SW_FLAG_LABEL_EQUIVALENCE: the paper's scan + analysis labeling (comparison variant, not the product path)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-baseline-L", type=int, default=4096)

@@ -53,8 +53,12 @@ enum { SW_INIT_ORDERED = 0, SW_INIT_RANDOM = 1 };
 enum {
     SW_FLAG_DEFAULT       = 0,
     SW_FLAG_FORCE_GENERIC = 1,  /* use the any-L reference kernels even where the tiled path applies     */
-    SW_FLAG_LAZY_LABELS   = 2   /* do not materialise canonical labels every sweep; flatten on demand
+    SW_FLAG_LAZY_LABELS   = 2,  /* do not materialise canonical labels every sweep; flatten on demand
                                    (sw_get_labels / sw_measure of cluster sizes).  Same results.        */
+    SW_FLAG_LABEL_EQUIVALENCE = 4 /* comparison variant, any L: label step (2) with the "Label Equivalence" scheme
+                                   the paper uses (scanning + analysis kernels iterated until the
+                                   scanning changes nothing; the host reads a flag every round).  Same results,
+                                   much slower; sw_stats.le_rounds_* count the rounds (the paper: about 8.6).   */
 };
 
 /* --- life cycle -------------------------------------------------------------------------------
@@ -125,6 +129,8 @@ typedef struct sw_stats {
     uint64_t kernel_launches;   /* kernels launched by this context so far                          */
     uint64_t device_bytes;      /* device memory in use by this context                             */
     uint64_t sweeps;            /* sweeps issued so far                                             */
+    uint64_t le_rounds_last;    /* SW_FLAG_LABEL_EQUIVALENCE: scanning + analysis rounds of the last sweep,   */
+    uint64_t le_rounds_total;   /* ... and of all sweeps so far (the last round of a sweep changes nothing)   */
 } sw_stats;
 int sw_get_stats(sw_ctx *ctx, sw_stats *out);
 /* Time the kernels of the NEXT sweeps individually with CUDA events on the context stream:

@@ -14,7 +14,7 @@ import numpy as np
 
 OK, ERR_INVALID_ARG, ERR_OOM, ERR_CUDA, ERR_STATE = 0, 1, 2, 3, 4
 INIT_ORDERED, INIT_RANDOM = 0, 1
-FLAG_DEFAULT, FLAG_FORCE_GENERIC, FLAG_LAZY_LABELS = 0, 1, 2
+FLAG_DEFAULT, FLAG_FORCE_GENERIC, FLAG_LAZY_LABELS, FLAG_LABEL_EQUIVALENCE = 0, 1, 2, 4
 MAX_KERNEL_SLOTS = 8
 _STATUS = {1: "SW_ERR_INVALID_ARG", 2: "SW_ERR_OOM", 3: "SW_ERR_CUDA", 4: "SW_ERR_STATE"}
 
@@ -40,7 +40,8 @@ class SwError(RuntimeError):
 class Stats(C.Structure):
     _fields_ = [("path", C.c_uint32), ("tile_w", C.c_uint32), ("tile_h", C.c_uint32),
                 ("kernels_per_sweep", C.c_uint32), ("kernel_launches", C.c_uint64),
-                ("device_bytes", C.c_uint64), ("sweeps", C.c_uint64)]
+                ("device_bytes", C.c_uint64), ("sweeps", C.c_uint64),
+                ("le_rounds_last", C.c_uint64), ("le_rounds_total", C.c_uint64)]
 
 
 def lib():

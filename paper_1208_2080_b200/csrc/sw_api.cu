@@ -36,7 +36,7 @@ struct Plan {
     size_t spins, bonds, labels, rootbits, border, edges, tile_clusters, row, flag, total;   // byte offsets into the workspace
 };
 
-bool tiled_ok(uint32_t L, uint32_t flags) { return (L % sw::kTile == 0) && !(flags & SW_FLAG_FORCE_GENERIC); }
+bool tiled_ok(uint32_t L, uint32_t flags) { return (L % sw::kTile == 0) && !(flags & (SW_FLAG_FORCE_GENERIC | SW_FLAG_LABEL_EQUIVALENCE)); }
 
 Plan make_plan(uint32_t L, uint32_t q, uint32_t flags)
 {
@@ -62,7 +62,8 @@ struct sw_ctx {
     uint32_t L = 0, q = 0, flags = 0;
     uint64_t N = 0, seed = 0, T = 0, t = 0;
     double K = 0;
-    bool tiled = false, lazy = false;
+    bool tiled = false, lazy = false, label_equiv = false;
+    uint64_t le_rounds_last = 0, le_rounds_total = 0;
     bool have_spins = false, have_labels = false, labels_flat = false;
     bool owns_ws = false, owns_stream = false;
     int device = 0;
@@ -166,6 +167,28 @@ int sweep_once(sw_ctx *c, bool count_clusters)
                               : (count_clusters ? sw::k_tile_flip<true, true, true> : sw::k_tile_flip<true, true, false>);
           flip<<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters); }
         c->labels_flat = !c->lazy;
+    } else if (c->label_equiv) {
+        // the loop of scanning and analysis kernels "is iterated up to the point when the information of
+        // the labeling needs no more process of scanning function"; as in the paper the host looks at a flag every round
+        const int th = 256;
+        { Timed tm(c, SLOT_G_BONDS);
+          sw::k_bonds_generic<<<grid_for(c, (c->N + 15) / 16, th), th, 0, c->stream>>>(c->d_spins, c->d_bonds, P); }
+        { Timed tm(c, SLOT_G_INIT);
+          sw::k_label_identity<<<grid_for(c, c->N, th), th, 0, c->stream>>>(c->d_labels, P); }
+        c->le_rounds_last = 0;
+        for (uint32_t changed = 1; changed;) {
+            SW_CUDA(c, cudaMemsetAsync(c->d_flag, 0, 4, c->stream));
+            c->launches += 2;
+            sw::k_le_scan<<<grid_for(c, c->N, th), th, 0, c->stream>>>(c->d_bonds, c->d_labels, P, c->d_flag);
+            sw::k_le_analysis<<<grid_for(c, c->N, th), th, 0, c->stream>>>(c->d_labels, P);
+            SW_CUDA(c, cudaMemcpyAsync(&changed, c->d_flag, 4, cudaMemcpyDeviceToHost, c->stream));
+            SW_CUDA(c, cudaStreamSynchronize(c->stream));
+            c->le_rounds_last += 1;
+        }
+        c->le_rounds_total += c->le_rounds_last;
+        { Timed tm(c, SLOT_G_FLIP);
+          sw::k_flip_generic<<<grid_for(c, c->N, th), th, 0, c->stream>>>(c->d_labels, c->d_spins, P); }
+        c->labels_flat = true;
     } else {
         const int th = 256;
         { Timed tm(c, SLOT_G_BONDS);
@@ -250,13 +273,14 @@ int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed,
     *out = nullptr;
     uint64_t T = 0;
     if (L < 2 || L > 65536 || q < 2 || q > 255 || !host_threshold(K, &T)) return SW_ERR_INVALID_ARG;
-    if (flags & ~(uint32_t)(SW_FLAG_FORCE_GENERIC | SW_FLAG_LAZY_LABELS)) return SW_ERR_INVALID_ARG;
+    if (flags & ~(uint32_t)(SW_FLAG_FORCE_GENERIC | SW_FLAG_LAZY_LABELS | SW_FLAG_LABEL_EQUIVALENCE)) return SW_ERR_INVALID_ARG;
     sw_ctx *c = new (std::nothrow) sw_ctx();
     if (!c) return SW_ERR_OOM;
     c->L = L; c->q = q; c->K = K; c->seed = seed; c->T = T; c->flags = flags;
     c->N = (uint64_t)L * L;
     c->tiled = tiled_ok(L, flags);
-    c->lazy = (flags & SW_FLAG_LAZY_LABELS) != 0;
+    c->label_equiv = (flags & SW_FLAG_LABEL_EQUIVALENCE) != 0;
+    c->lazy = (flags & SW_FLAG_LAZY_LABELS) != 0 && !c->label_equiv;   // the analysis kernel leaves flat labels anyway
     const Plan plan = make_plan(L, q, flags);
     cudaError_t e = cudaGetDevice(&c->device);
     if (e != cudaSuccess) { delete c; return SW_ERR_CUDA; }
@@ -479,10 +503,12 @@ int sw_get_stats(sw_ctx *c, sw_stats *out)
     if (!c || !out) return SW_ERR_INVALID_ARG;
     out->path = c->tiled ? 1u : 0u;
     out->tile_w = out->tile_h = c->tiled ? sw::kTile : 0u;
-    out->kernels_per_sweep = c->tiled ? 3u : (c->lazy ? 4u : 5u);
+    out->kernels_per_sweep = c->tiled ? 3u : c->label_equiv ? (uint32_t)(3u + 2u * c->le_rounds_last) : (c->lazy ? 4u : 5u);
     out->kernel_launches = c->launches;
     out->device_bytes = c->ws_bytes + (c->d_sizes ? c->N * 4 : 0);
     out->sweeps = c->sweeps;
+    out->le_rounds_last = c->le_rounds_last;
+    out->le_rounds_total = c->le_rounds_total;
     return SW_OK;
 }
 
@@ -516,6 +542,7 @@ const char *sw_kernel_name(sw_ctx *c, int slot)
     const bool tiled_slot = slot <= SLOT_FLIP;
     if (tiled_slot != c->tiled) return nullptr;
     if (slot == SLOT_G_FLATTEN && c->lazy) return nullptr;
+    if (c->label_equiv && (slot == SLOT_G_UNION || slot == SLOT_G_FLATTEN)) return nullptr;   // scan / analysis rounds are not timed per slot
     return kSlotNames[slot];
 }
 

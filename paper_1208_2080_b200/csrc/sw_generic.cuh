@@ -86,6 +86,46 @@ __global__ void k_union_generic(const uint32_t *__restrict__ bonds, uint32_t *la
     }
 }
 
+// --- comparison variant: "Label Equivalence" of Kalentev et al., as the paper describes it -------
+// SW_FLAG_LABEL_EQUIVALENCE.  Prior art, kept behind the same ABI to reproduce the one per-step figure the paper
+// gives (about 8.6 scan + analysis rounds per sweep at 4096^2, q = 2, T_c) and to show what the tiled path buys.
+//
+// scanning: "compares the label of each site with that of the nearest-neighbor sites when the bond between [them] is
+// active.  If the label of the nearest-neighbor site is smaller than the label of that site, the label variable with
+// the label number, label[label], is updated to the smallest one."  All four neighbours are looked at (a site owns its
+// right and down bond; the left and up bonds belong to the neighbours).  *changed is set if anything was lowered.
+__global__ void k_le_scan(const uint32_t *__restrict__ bonds, uint32_t *labels, Params P, uint32_t *changed)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    const uint64_t L = P.L;
+    bool any = false;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += stride) {
+        const uint64_t y = i / L, x = i - y * L;
+        const uint64_t ir = y * L + (x + 1 == L ? 0 : x + 1), id = (y + 1 == L ? 0 : y + 1) * L + x;
+        const uint64_t il = y * L + (x == 0 ? L - 1 : x - 1), iu = (y == 0 ? L - 1 : y - 1) * L + x;
+        const uint32_t wi = bonds[i >> 4], wl = bonds[il >> 4], wu = bonds[iu >> 4];
+        const uint32_t mine = ld_label(labels, (uint32_t)i);
+        uint32_t m = mine;
+        if ((wi >> (i & 15)) & 1u) m = min(m, ld_label(labels, (uint32_t)ir));
+        if ((wi >> (16 + (i & 15))) & 1u) m = min(m, ld_label(labels, (uint32_t)id));
+        if ((wl >> (il & 15)) & 1u) m = min(m, ld_label(labels, (uint32_t)il));
+        if ((wu >> (16 + (iu & 15))) & 1u) m = min(m, ld_label(labels, (uint32_t)iu));
+        if (m < mine) { atomicMin(labels + mine, m); any = true; }
+    }
+    if (__any_sync(0xFFFFFFFFu, any) && (threadIdx.x & 31) == 0) atomicOr(changed, 1u);
+}
+
+// analysis: "each thread tracks back the label variable until the label variable, label, remains unchanged."
+__global__ void k_le_analysis(uint32_t *labels, Params P)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += stride) {
+        uint32_t l = ld_label(labels, (uint32_t)i), r = ld_label(labels, l);
+        while (r != l) { l = r; r = ld_label(labels, l); }
+        labels[i] = l;
+    }
+}
+
 // labels[i] <- root(i).  In-place is safe: whatever another thread reads is an ancestor.
 __global__ void k_flatten_generic(uint32_t *labels, Params P)
 {
