@@ -128,7 +128,7 @@ constexpr int kFlipRows = 2 * kFlipAcc;                          // tile rows pe
 // kSpins: draw and write the new spins; kCount: leave the number of canonical roots per warp in tile_clusters[]
 // (n_clusters of sw_measure without a pass over labels[]; costs 3 % of the kernel, so only the last sweep of a call does it).
 template <bool kLabels, bool kSpins, bool kCount>
-__global__ void __launch_bounds__(kFlipThreads, 5)
+__global__ void __launch_bounds__(kFlipThreads, 6)
 k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__restrict__ spins, Params P,
             uint32_t *__restrict__ tile_clusters)
 {
@@ -148,19 +148,28 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
     // -- phase A: everything this tile needs from HBM is requested at once: my labels and root flags.
     //    A tile-local root's own entry is its link into the global forest (itself if the merge never hooked
     //    it), so the first step of every chase comes out of this coalesced load instead of a scattered one.
-    uint32_t lab[4 * kFlipAcc];
+    //    What a site needs afterwards is the tile-local id of its root (12 bits; its own id if it is a root): two per
+    //    register, so the 16 sites of a thread cost 8 registers across the chases instead of 16.
+    uint32_t ids[2 * kFlipAcc];
     uint32_t work = 0;                                         // bit 4k + j: my site j of access k is a tile-local root
 #pragma unroll
     for (int k = 0; k < kFlipAcc; ++k) {
         const uint32_t i0 = i00 + 2 * k * L;
         const uint4 l = __ldcg(reinterpret_cast<const uint4 *>(labels + i0));
-        lab[4 * k] = l.x; lab[4 * k + 1] = l.y; lab[4 * k + 2] = l.z; lab[4 * k + 3] = l.w;
-        const uint32_t rb = rootbits[i0 >> 4];
-        work |= ((rb >> (x4 & 12u)) & 15u) << (4 * k);
-    }
+        const uint32_t lab[4] = {l.x, l.y, l.z, l.w};
+        const uint32_t rb = (rootbits[i0 >> 4] >> (x4 & 12u)) & 15u;
+        const uint32_t id0 = ((yk0 + 2 * k) << 6) + x4;
+        uint32_t id[4];
 #pragma unroll
-    for (int j = 0; j < 4 * kFlipAcc; ++j)
-        if ((work >> j) & 1u) s_root[((yk0 + 2 * (j >> 2)) << 6) + x4 + (j & 3)] = lab[j];
+        for (int j = 0; j < 4; ++j) {
+            const bool isroot = (rb >> j) & 1u;
+            if (isroot) s_root[id0 + j] = lab[j];              // where the chase of this root starts
+            id[j] = isroot ? id0 + j : lab[j];
+        }
+        ids[2 * k] = id[0] | (id[1] << 16);
+        ids[2 * k + 1] = id[2] | (id[3] << 16);
+        work |= rb << (4 * k);
+    }
 
     {
         // each warp lists the tile-local roots of its rows (prefix sum over the lanes, no atomics) ...
@@ -196,19 +205,17 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
 #pragma unroll
     for (int k = 0; k < kFlipAcc; ++k) {
         const uint32_t i0 = i00 + 2 * k * L;
-        const uint32_t id0 = ((yk0 + 2 * k) << 6) + x4;
-        uint32_t st = 0;
+        uint32_t st = 0, lab[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const bool isroot = (work >> (4 * k + j)) & 1u;     // a tile-local root stands for itself
-            const uint32_t id = isroot ? id0 + j : lab[4 * k + j];
-            lab[4 * k + j] = s_root[id];
-            if (kCount) canon += (lab[4 * k + j] == i0 + j);    // a canonical root is its own label
+            const uint32_t id = (j & 1) ? ids[2 * k + (j >> 1)] >> 16 : ids[2 * k + (j >> 1)] & 0xFFFFu;
+            lab[j] = s_root[id];
+            if (kCount) canon += (lab[j] == i0 + j);           // a canonical root is its own label
             if (kSpins) st |= (uint32_t)s_state[id] << (8 * j);
         }
         if (kSpins) *reinterpret_cast<uint32_t *>(spins + i0) = st;
         if (kLabels)
-            *reinterpret_cast<uint4 *>(labels + i0) = make_uint4(lab[4 * k], lab[4 * k + 1], lab[4 * k + 2], lab[4 * k + 3]);
+            *reinterpret_cast<uint4 *>(labels + i0) = make_uint4(lab[0], lab[1], lab[2], lab[3]);
     }
     if (kCount) {
         canon = __reduce_add_sync(0xFFFFFFFFu, canon);
