@@ -104,14 +104,18 @@ __device__ __forceinline__ uint32_t find_root_halving_from(uint32_t *labels, uin
 // target with b.  One pass over all bonds yields the complete partition (no outer iteration).
 __device__ __forceinline__ void unite(uint32_t *labels, uint32_t a, uint32_t b)
 {
+    {   // the first hop of both chases is loaded together: the common case (both are roots) costs one round trip, not two
+        const uint32_t pa = ld_label(labels, a), pb = ld_label(labels, b);
+        a = find_root_halving_from(labels, a, pa);
+        b = find_root_halving_from(labels, b, pb);
+    }
     while (true) {
-        a = find_root_halving(labels, a);
-        b = find_root_halving(labels, b);
         if (a == b) return;
         if (a < b) { const uint32_t s = a; a = b; b = s; }
         const uint32_t old = atomicMin(labels + a, b);
         if (old == a) return;
-        a = old;
+        a = find_root_halving(labels, old);
+        b = find_root_halving(labels, b);
     }
 }
 
