@@ -99,6 +99,14 @@ __device__ __forceinline__ uint32_t hclose(uint32_t n, uint32_t A, uint32_t A2, 
     return n;
 }
 
+// mask * 2 + (draw >= T): add.cc sets the carry iff draw + (2^32 - T) overflows, addc shifts it into the mask
+__device__ __forceinline__ uint32_t shift_in_not_below(uint32_t mask, uint32_t draw, uint32_t above)
+{
+    uint32_t t, out;
+    asm("add.cc.u32 %0, %2, %3;\n\taddc.u32 %1, %4, %4;" : "=r"(t), "=r"(out) : "r"(draw), "r"(above), "r"(mask));
+    return out;
+}
+
 // the four plane bytes of block row r as one word (byte b = plane b)
 __device__ __forceinline__ uint32_t plane_row(uint32_t P0, uint32_t P1, uint32_t P2, uint32_t P3, uint32_t r)
 {
@@ -166,6 +174,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
 
     // -- step (1): a bond is active iff the spins are equal and its draw is below the threshold
     uint32_t R = 0, D = 0;
+    const uint32_t above = ~P.thr_m1;                          // 2^32 - T (T >= 1; T = 0 is masked by thr_any)
     {
         // (a rolled loop over the four rows with the rows rotating through registers: the unrolled body is four times
         //  the code, and with 32 warps in different phases of this kernel the instruction cache is what runs out)
@@ -177,15 +186,19 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
             const uint32_t eq_r = pack4(__vcmpeq4(a0, n0)) | (pack4(__vcmpeq4(a1, n1)) << 4);
             const uint32_t eq_d = pack4(__vcmpeq4(a0, n1r.x)) | (pack4(__vcmpeq4(a1, n1r.y)) << 4);
             const uint32_t pair0 = (i0 + r * L) >> 1;
-            uint32_t m_r = 0, m_d = 0;
+            // threshold tests as carry chains: draw + (2^32 - T) carries out iff draw >= T, and "shift the mask left,
+            // insert the carry" is an add with carry-in: two ALU instructions per bond instead of compare + select + or.
+            // Pairs run from the last to the first so the bits land in order; the mask collects the INACTIVE draws.
+            uint32_t off_r = 0, off_d = 0;
 #pragma unroll
-            for (int p = 0; p < 4; ++p) {                      // one Philox call per site pair: right, down, right, down
+            for (int p = 3; p >= 0; --p) {                     // one Philox call per site pair: right, down, right, down
                 const uint4 d = philox4x32_10(pair0 + p, 0u, P.t, kPurposeBond, P);
-                m_r |= (uint32_t)(d.x <= P.thr_m1) << (2 * p);
-                m_d |= (uint32_t)(d.y <= P.thr_m1) << (2 * p);
-                m_r |= (uint32_t)(d.z <= P.thr_m1) << (2 * p + 1);
-                m_d |= (uint32_t)(d.w <= P.thr_m1) << (2 * p + 1);
+                off_r = shift_in_not_below(off_r, d.z, above);
+                off_d = shift_in_not_below(off_d, d.w, above);
+                off_r = shift_in_not_below(off_r, d.x, above);
+                off_d = shift_in_not_below(off_d, d.y, above);
             }
+            const uint32_t m_r = ~off_r, m_d = ~off_d;
             R |= (eq_r & m_r) << (8 * r);
             D |= (eq_d & m_d) << (8 * r);
             cur = n1r; n1r = n2r; n2r = n3r; n3r = n4r;
