@@ -33,7 +33,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Plan {
-    size_t spins, bonds, labels, rootbits, border, edges, tile_clusters, row, flag, total;   // byte offsets into the workspace
+    size_t spins, bonds, labels, rootbits, border, edges, tile_clusters, draws, row, flag, total;   // byte offsets into the workspace
 };
 
 bool tiled_ok(uint32_t L, uint32_t flags) { return (L % sw::kTile == 0) && !(flags & (SW_FLAG_FORCE_GENERIC | SW_FLAG_LABEL_EQUIVALENCE)); }
@@ -50,6 +50,7 @@ Plan make_plan(uint32_t L, uint32_t q, uint32_t flags)
     p.border = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileBorder) : 0));
     p.edges = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileEdges) : 0));
     p.tile_clusters = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * (sw::kFlipThreads / 32) * 4 : 0));
+    p.draws = off;  off = align_up(off + (tiled_ok(L, flags) ? (N / 32) * sizeof(uint2) : 0));   // one uint2 per 8 x 4 block
     p.row = off;    off = align_up(off + (3 + (size_t)q) * 8);
     p.flag = off;   off = align_up(off + 4);
     p.total = off;
@@ -72,6 +73,8 @@ struct sw_ctx {
     size_t ws_bytes = 0;
     uint8_t *d_spins = nullptr;
     uint32_t *d_bonds = nullptr, *d_labels = nullptr, *d_flag = nullptr, *d_tile_clusters = nullptr;
+    uint2 *d_draws = nullptr;             // bond-draw masks of sweep draws_t (tiled path), made one sweep ahead
+    uint64_t draws_t = ~0ull;
     uint16_t *d_rootbits = nullptr;
     sw::TileBorder *d_border = nullptr;
     sw::TileEdges *d_edges = nullptr;
@@ -158,14 +161,19 @@ int sweep_once(sw_ctx *c, bool count_clusters)
     const Params P = make_params(c, c->t);
     if (c->tiled) {
         const unsigned tiles = (unsigned)(c->N / sw::kTileSites);
+        if (c->draws_t != c->t) {        // first sweep after sw_init / sw_set_state: nobody has made this sweep's bond draws yet
+            c->launches += 1;
+            sw::k_draws<<<tiles, 256, 0, c->stream>>>(c->d_draws, P);
+        }
         { Timed tm(c, SLOT_TILE);
-          sw::k_tile_blocks<<<tiles, sw::kBlkThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_edges, P); }
+          sw::k_tile_blocks<<<tiles, sw::kBlkThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_edges, c->d_draws, P); }
         { Timed tm(c, SLOT_MERGE);
           sw::k_tile_merge<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_edges, P, tiles); }
         { Timed tm(c, SLOT_FLIP);
           auto flip = c->lazy ? (count_clusters ? sw::k_tile_flip<false, true, true> : sw::k_tile_flip<false, true, false>)
                               : (count_clusters ? sw::k_tile_flip<true, true, true> : sw::k_tile_flip<true, true, false>);
-          flip<<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters); }
+          flip<<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, c->d_draws); }
+        c->draws_t = c->t + 1;           // the flip kernel made the draws of the next sweep on the side
         c->labels_flat = !c->lazy;
     } else if (c->label_equiv) {
         // the loop of scanning and analysis kernels "is iterated up to the point when the information of
@@ -217,7 +225,7 @@ int ensure_flat(sw_ctx *c)
     const Params P = make_params(c, c->t);
     c->launches += 1;
     if (c->tiled)       // lazy mode: the forest of the last sweep is still in place (tile-local ids + root links)
-        sw::k_tile_flip<true, false, false><<<(unsigned)(c->N / sw::kTileSites), sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters);
+        sw::k_tile_flip<true, false, false><<<(unsigned)(c->N / sw::kTileSites), sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, nullptr);
     else
         sw::k_flatten_generic<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_labels, P);
     SW_CUDA(c, cudaGetLastError());
@@ -302,6 +310,7 @@ int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed,
     c->d_border = (sw::TileBorder *)(c->ws + plan.border);
     c->d_edges = (sw::TileEdges *)(c->ws + plan.edges);
     c->d_tile_clusters = (uint32_t *)(c->ws + plan.tile_clusters);
+    c->d_draws = (uint2 *)(c->ws + plan.draws);
     c->d_row = (unsigned long long *)(c->ws + plan.row);
     c->d_flag = (uint32_t *)(c->ws + plan.flag);
     *out = c;

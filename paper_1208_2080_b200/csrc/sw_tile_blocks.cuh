@@ -99,14 +99,6 @@ __device__ __forceinline__ uint32_t hclose(uint32_t n, uint32_t A, uint32_t A2, 
     return n;
 }
 
-// mask * 2 + (draw >= T): add.cc sets the carry iff draw + (2^32 - T) overflows, addc shifts it into the mask
-__device__ __forceinline__ uint32_t shift_in_not_below(uint32_t mask, uint32_t draw, uint32_t above)
-{
-    uint32_t t, out;
-    asm("add.cc.u32 %0, %2, %3;\n\taddc.u32 %1, %4, %4;" : "=r"(t), "=r"(out) : "r"(draw), "r"(above), "r"(mask));
-    return out;
-}
-
 // the four plane bytes of block row r as one word (byte b = plane b)
 __device__ __forceinline__ uint32_t plane_row(uint32_t P0, uint32_t P1, uint32_t P2, uint32_t P3, uint32_t r)
 {
@@ -127,7 +119,7 @@ __device__ __forceinline__ uint32_t slot_of4(uint32_t W, uint32_t c)
 __global__ void __launch_bounds__(kBlkThreads, 8)
 k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
               uint32_t *__restrict__ labels, uint16_t *__restrict__ rootbits,
-              TileBorder *__restrict__ border, TileEdges *__restrict__ edges, Params P)
+              TileBorder *__restrict__ border, TileEdges *__restrict__ edges, const uint2 *__restrict__ draws, Params P)
 {
     __shared__ BlkShared S;
 
@@ -174,35 +166,22 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
 
     // -- step (1): a bond is active iff the spins are equal and its draw is below the threshold
     uint32_t R = 0, D = 0;
-    const uint32_t above = ~P.thr_m1;                          // 2^32 - T (T >= 1; T = 0 is masked by thr_any)
     {
-        // (a rolled loop over the four rows with the rows rotating through registers: the unrolled body is four times
-        //  the code, and with 32 warps in different phases of this kernel the instruction cache is what runs out)
-        uint2 cur = s[0], n1r = s[1], n2r = s[2], n3r = s[3], n4r = s[4];
-#pragma unroll 1
+        // The threshold tests of this sweep's draws were made ahead of time (tile_draw_masks in sw_tiled.cuh: by the flip
+        // kernel of the previous sweep while it waited for its loads, or by k_draws): bit 8r + c of dm.x / dm.y says
+        // whether the right / down draw of my site (r, c) is below the threshold.
+        const uint2 dm = draws[blockIdx.x * kBlkThreads + tid];
+#pragma unroll
         for (int r = 0; r < 4; ++r) {
-            const uint32_t a0 = cur.x, a1 = cur.y;
+            const uint32_t a0 = s[r].x, a1 = s[r].y;
             const uint32_t n0 = __funnelshift_r(a0, a1, 8), n1 = __funnelshift_r(a1, nx >> (8 * r), 8);
             const uint32_t eq_r = pack4(__vcmpeq4(a0, n0)) | (pack4(__vcmpeq4(a1, n1)) << 4);
-            const uint32_t eq_d = pack4(__vcmpeq4(a0, n1r.x)) | (pack4(__vcmpeq4(a1, n1r.y)) << 4);
-            const uint32_t pair0 = (i0 + r * L) >> 1;
-            // threshold tests as carry chains: draw + (2^32 - T) carries out iff draw >= T, and "shift the mask left,
-            // insert the carry" is an add with carry-in: two ALU instructions per bond instead of compare + select + or.
-            // Pairs run from the last to the first so the bits land in order; the mask collects the INACTIVE draws.
-            uint32_t off_r = 0, off_d = 0;
-#pragma unroll
-            for (int p = 3; p >= 0; --p) {                     // one Philox call per site pair: right, down, right, down
-                const uint4 d = philox4x32_10(pair0 + p, 0u, P.t, kPurposeBond, P);
-                off_r = shift_in_not_below(off_r, d.z, above);
-                off_d = shift_in_not_below(off_d, d.w, above);
-                off_r = shift_in_not_below(off_r, d.x, above);
-                off_d = shift_in_not_below(off_d, d.y, above);
-            }
-            const uint32_t m_r = ~off_r, m_d = ~off_d;
-            R |= (eq_r & m_r) << (8 * r);
-            D |= (eq_d & m_d) << (8 * r);
-            cur = n1r; n1r = n2r; n2r = n3r; n3r = n4r;
+            const uint32_t eq_d = pack4(__vcmpeq4(a0, s[r + 1].x)) | (pack4(__vcmpeq4(a1, s[r + 1].y)) << 4);
+            R |= eq_r << (8 * r);
+            D |= eq_d << (8 * r);
         }
+        R &= dm.x;
+        D &= dm.y;
     }
     R &= P.thr_any;
     D &= P.thr_any;

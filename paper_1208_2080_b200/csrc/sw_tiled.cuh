@@ -41,6 +41,55 @@ struct __align__(16) TileEdges {
 // the four 0x00/0xFF bytes of a __vcmpeq4 result -> 4 bits
 __device__ __forceinline__ uint32_t pack4(uint32_t eq) { return ((eq & 0x01010101u) * 0x01020408u) >> 24; }
 
+// ---- bond draws, made ahead of time ------------------------------------------------------------
+// Whether a bond's draw is below the threshold depends on (seed, sweep, site) only, not on the spins (counter-based
+// Philox, R11), so the tests of sweep t + 1 can be made while sweep t is still running.  The tile kernel is
+// bound by its integer ALU pipe and a quarter of its instructions were these draws; the flip kernel waits for HBM and
+// has the issue slots to spare.  One uint2 per 8 x 4 block of the tile kernel (index tile * 128 + block): bit 8r + c
+// of .x / .y = the right / down draw of site (r, c) of the block is below the threshold.
+
+// mask * 2 + (draw >= T): add.cc sets the carry iff draw + (2^32 - T) overflows, addc shifts it into the mask
+__device__ __forceinline__ uint32_t shift_in_not_below(uint32_t mask, uint32_t draw, uint32_t above)
+{
+    uint32_t t, out;
+    asm("add.cc.u32 %0, %2, %3;\n\taddc.u32 %1, %4, %4;" : "=r"(t), "=r"(out) : "r"(draw), "r"(above), "r"(mask));
+    return out;
+}
+
+// 256 threads per tile: thread u makes the draws of rows 2h, 2h + 1 (h = u % 2) of block u / 2: one Philox call per
+// site pair (words: right, down, right, down), last pair first so that the bits are shifted in in order.
+__device__ __forceinline__ void tile_draw_masks(uint2 *__restrict__ draws, uint32_t tile, uint32_t origin, uint32_t u,
+                                                uint32_t t, const Params &P)
+{
+    const uint32_t b = u >> 1, h = u & 1u, bx = b & 7u, by = b >> 3;
+    const uint32_t above = ~P.thr_m1;                          // 2^32 - T (T >= 1; T = 0 is masked by thr_any)
+    uint32_t off_r = 0, off_d = 0;                             // the draws that are NOT below the threshold
+#pragma unroll
+    for (int rr = 1; rr >= 0; --rr) {
+        const uint32_t pair0 = (origin + ((by << 2) + 2u * h + rr) * P.L + (bx << 3)) >> 1;
+#pragma unroll
+        for (int p = 3; p >= 0; --p) {
+            const uint4 d = philox4x32_10(pair0 + p, 0u, t, kPurposeBond, P);
+            off_r = shift_in_not_below(off_r, d.z, above);
+            off_d = shift_in_not_below(off_d, d.w, above);
+            off_r = shift_in_not_below(off_r, d.x, above);
+            off_d = shift_in_not_below(off_d, d.y, above);
+        }
+    }
+    const uint32_t m_r = ~off_r & 0xFFFFu & P.thr_any, m_d = ~off_d & 0xFFFFu & P.thr_any;
+    const uint32_t o_r = __shfl_xor_sync(0xFFFFFFFFu, m_r, 1), o_d = __shfl_xor_sync(0xFFFFFFFFu, m_d, 1);
+    if (h == 0) draws[tile * 128u + b] = make_uint2(m_r | (o_r << 16), m_d | (o_d << 16));
+}
+
+// the draws of sweep P.t for every tile (first sweep after sw_init / sw_set_state; later ones come from k_tile_flip)
+__global__ void __launch_bounds__(256)
+k_draws(uint2 *__restrict__ draws, Params P)
+{
+    const uint32_t tiles_x = P.L >> 6;
+    const uint32_t ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
+    tile_draw_masks(draws, blockIdx.x, (ty << 6) * P.L + (tx << 6), threadIdx.x, P.t, P);
+}
+
 // ---- kernel 2: merge across tile borders -------------------------------------------------------
 // One thread per border site (64 on the right column, 64 on the bottom row of a tile).  Only about a
 // third of them carry a link worth uniting (active bond, not a repeat of its neighbour's link), and a
@@ -120,7 +169,7 @@ k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, const Tile
 // its k-th access covers rows kFlipRows w + 2k and + 2k + 1; lane l holds the 4 sites
 // x = 4 (l % 16) .. + 3 of row kFlipRows w + 2k + l / 16.
 
-constexpr int kFlipThreads = 256;
+constexpr int kFlipThreads = 256;                                // (tile_draw_masks is written for 256 threads per tile)
 constexpr int kFlipAcc = (int)kTileSites / (4 * kFlipThreads);   // 16-byte accesses per thread
 constexpr int kFlipRows = 2 * kFlipAcc;                          // tile rows per warp
 
@@ -130,7 +179,7 @@ constexpr int kFlipRows = 2 * kFlipAcc;                          // tile rows pe
 template <bool kLabels, bool kSpins, bool kCount>
 __global__ void __launch_bounds__(kFlipThreads, 6)
 k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__restrict__ spins, Params P,
-            uint32_t *__restrict__ tile_clusters)
+            uint32_t *__restrict__ tile_clusters, uint2 *__restrict__ next_draws)
 {
     __shared__ uint32_t s_root[kTileSites];                   // per tile-local root: its canonical root
     __shared__ uint8_t s_state[kTileSites];                   // per tile-local root: the new state
@@ -152,12 +201,21 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
     //    register, so the 16 sites of a thread cost 8 registers across the chases instead of 16.
     uint32_t ids[2 * kFlipAcc];
     uint32_t work = 0;                                         // bit 4k + j: my site j of access k is a tile-local root
+    uint4 lq[kFlipAcc];
+    uint32_t rq[kFlipAcc];
 #pragma unroll
     for (int k = 0; k < kFlipAcc; ++k) {
         const uint32_t i0 = i00 + 2 * k * L;
-        const uint4 l = __ldcg(reinterpret_cast<const uint4 *>(labels + i0));
+        lq[k] = __ldcg(reinterpret_cast<const uint4 *>(labels + i0));
+        rq[k] = rootbits[i0 >> 4];
+    }
+    // while those loads are on their way: the bond draws of the NEXT sweep for this tile (pure arithmetic, see above)
+    if (kSpins && next_draws) tile_draw_masks(next_draws, blockIdx.x, origin, tid, P.t + 1u, P);
+#pragma unroll
+    for (int k = 0; k < kFlipAcc; ++k) {
+        const uint4 l = lq[k];
         const uint32_t lab[4] = {l.x, l.y, l.z, l.w};
-        const uint32_t rb = (rootbits[i0 >> 4] >> (x4 & 12u)) & 15u;
+        const uint32_t rb = (rq[k] >> (x4 & 12u)) & 15u;
         const uint32_t id0 = ((yk0 + 2 * k) << 6) + x4;
         uint32_t id[4];
 #pragma unroll

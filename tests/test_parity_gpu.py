@@ -132,7 +132,7 @@ def test_tiled_path_is_selected_and_counts_kernels():
     g.synchronize()
     st = g.stats()
     assert st["path"] == 1 and (st["tile_w"], st["tile_h"]) == (64, 64) and st["kernels_per_sweep"] == 3
-    assert st["kernel_launches"] == 9 and st["sweeps"] == 3
+    assert st["kernel_launches"] == 10 and st["sweeps"] == 3   # k_draws once + 3 per sweep
 
 
 def test_q255_and_large_seed():
