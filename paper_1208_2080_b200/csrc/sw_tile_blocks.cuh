@@ -31,11 +31,13 @@ constexpr int kBlkExtraCap = 32 * 11;         // per warp: <= 7 up-links + 4 lef
 constexpr uint32_t kDecodeMul = (1u << 24) | (1u << 17) | (1u << 10) | (1u << 3);
 
 struct BlkShared {
-    uint16_t parent[kTileSites];              // union-find over tile-local site ids (y * 64 + x); only component seeds are linked
+    uint16_t parent[kTileSites];              // union-find over tile-local site ids (y * 64 + x): component seeds are linked; a site of
+                                              // the right column of a block points at its seed (the block on its right links to the site)
     uint32_t list[kBlkSlots][kBlkThreads];    // per thread, slot k: component mask -> seed id | seed bit << 16 -> global label of its root
     uint16_t pub_bottom[8][kBlkThreads];      // seed id of the component of my bottom-row site c
-    uint16_t pub_right[4][kBlkThreads];       // seed id of the component of my right-column site r
-    uint32_t R[kBlkThreads], D[kBlkThreads];  // right / down bond masks of every block (bit 8r+7 / 24+c leave the block)
+    uint32_t edge[kBlkThreads];               // what the blocks below / to the right need to know about a block: bits 0-7 down
+                                              // bonds of row 3, 8-15 right bonds of row 3, 16-19 right bonds of column 7,
+                                              // 20-22 down bonds of column 7 (rows 0-2)
     uint32_t n_extra[kBlkThreads / 32];
 };
 // The links that need the atomic pass are buffered per warp in list slots kBlkBufSlot .. kBlkSlots-1, which are
@@ -116,7 +118,7 @@ __device__ __forceinline__ uint32_t slot_of4(uint32_t W, uint32_t c)
     return (((W >> c) & 0x01010101u) * kDecodeMul) >> 24;
 }
 
-__global__ void __launch_bounds__(kBlkThreads, 8)
+__global__ void __launch_bounds__(kBlkThreads, 9)
 k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
               uint32_t *__restrict__ labels, uint16_t *__restrict__ rootbits,
               TileBorder *__restrict__ border, TileEdges *__restrict__ edges, const uint2 *__restrict__ draws, Params P)
@@ -185,8 +187,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
     }
     R &= P.thr_any;
     D &= P.thr_any;
-    S.R[tid] = R;
-    S.D[tid] = D;
+    S.edge[tid] = (D >> 24) | ((R >> 24) << 8) | (pack4((R >> 7) & 0x01010101u) << 16) | (pack4((D >> 7) & 0x00010101u) << 20);
 
     // bond words cover 16 sites = my row and my lane-pair partner's: the even lane stores rows 0-1, the odd lane rows 2-3
     const uint32_t odd = bx & 1u;
@@ -200,13 +201,12 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
             bonds[(i0 + r * L) >> 4] = word;
         }
     }
-    __syncthreads();                                           // B1: parent[], R[], D[] visible
+    __syncthreads();                                           // B1: parent[], edge[] visible
 
     // -- the bonds that leave the tile (warp 0): right bonds of block column 7, down bonds of block row 15
     if (warp == 0) {
-        const uint32_t rc = S.R[((lane & 15u) << 3) + 7u];                            // block (7, lane): rows 4 lane .. 4 lane + 3
-        const uint32_t nib = (((rc >> 7) & 0x01010101u) * 0x01020408u) >> 24;         // bit r = its right bond of row r
-        const uint32_t dn = S.D[120u + (lane & 7u)] >> 24;                            // block (lane, 15): columns 8 lane .. + 7
+        const uint32_t nib = (S.edge[((lane & 15u) << 3) + 7u] >> 16) & 15u;          // block (7, lane): bit r = right bond of its row r
+        const uint32_t dn = S.edge[120u + (lane & 7u)] & 0xFFu;                       // block (lane, 15): down bonds of columns 8 lane .. + 7
         const uint32_t r_lo = __reduce_or_sync(0xFFFFFFFFu, lane < 8u ? nib << (4u * lane) : 0u);
         const uint32_t r_hi = __reduce_or_sync(0xFFFFFFFFu, (lane >= 8u && lane < 16u) ? nib << (4u * (lane - 8u)) : 0u);
         const uint32_t b_lo = __reduce_or_sync(0xFFFFFFFFu, lane < 4u ? dn << (8u * lane) : 0u);
@@ -225,8 +225,9 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
     const uint32_t Dl = D & 0x00FFFFFFu;                       // bit j: bond j -- j+8 inside the block
     const uint32_t Ds = Dl << 8;
     // links to other blocks of the tile, as masks over MY sites
-    const uint32_t up_row3 = by > 0u ? S.D[tid - 8u] >> 24 : 0u;                      // bit c: (block above, row 3, c) -- my (0, c)
-    const uint32_t left_c7 = bx > 0u ? (S.R[tid - 1u] >> 7) & 0x01010101u : 0u;       // bit 8r: (left block, r, 7) -- my (r, 0)
+    const uint32_t e_up = by > 0u ? S.edge[tid - 8u] : 0u, e_left = bx > 0u ? S.edge[tid - 1u] : 0u;
+    const uint32_t up_row3 = e_up & 0xFFu;                                            // bit c: (block above, row 3, c) -- my (0, c)
+    const uint32_t left_c7 = (((e_left >> 16) & 15u) * 0x00204081u) & 0x01010101u;    // bit 8r: (left block, r, 7) -- my (r, 0)
     const uint32_t out = (by < 15u ? D & 0xFF000000u : 0u) | (bx < 7u ? R & 0x80808080u : 0u);
     // sites that belong to a component worth a slot: any bond inside the block, or a link to another block
     const uint32_t todo = A | (A << 1) | Dl | Ds | up_row3 | left_c7 | out;
@@ -270,7 +271,9 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
         }
     }
 
-    // -- publish the seeds of my bottom row and right column for the blocks below / to the right
+    // -- publish the seeds of my bottom row for the block below (its up-links become plain-store parents); the sites
+    //    of my right column point at the seed of their component, and the block on my right links to those SITES
+    //    (one more hop in its finds; those links go through the atomic pass anyway)
     {
         const uint32_t W3 = plane_row(P0, P1, P2, P3, 3u), V3 = (P4 >> 24) << 4;
 #pragma unroll
@@ -279,7 +282,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
             const uint32_t Wr = plane_row(P0, P1, P2, P3, r), Vr = ((P4 >> (8 * r)) & 0xFFu) << 4;
-            S.pub_right[r][tid] = (uint16_t)S.list[slot_of(Wr, Vr, 7u)][tid];
+            if ((todo >> (8 * r + 7)) & 1u) S.parent[idbase + (r << 6) + 7u] = (uint16_t)S.list[slot_of(Wr, Vr, 7u)][tid];
         }
     }
 
@@ -289,7 +292,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
     auto walk_links = [&](auto &&on_first, auto &&on_other) {
         if (up_row3) {
             const uint32_t W0 = plane_row(P0, P1, P2, P3, 0u), V0 = (P4 & 0xFFu) << 4;
-            const uint32_t R_up = S.R[tid - 8u] >> 24;
+            const uint32_t R_up = (e_up >> 8) & 0xFFu;
             uint32_t u = up_row3 & ~((up_row3 & A & R_up & 0x7Fu) << 1);
             uint32_t seen = 0;
             while (u) {
@@ -306,13 +309,13 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
             }
         }
         if (left_c7) {
-            const uint32_t D_left = (S.D[tid - 1u] >> 7) & 0x00010101u;
+            const uint32_t D_left = (((e_left >> 20) & 7u) * 0x00204081u) & 0x00010101u;
             uint32_t l = left_c7 & ~((left_c7 & Dl & D_left) << 8);
             while (l) {
                 const uint32_t j = __ffs(l) - 1u, r = j >> 3;
                 l &= l - 1u;
                 const uint32_t Wr = plane_row(P0, P1, P2, P3, r), Vr = ((P4 >> j) & 0xFFu) << 4;
-                on_other(S.list[slot_of(Wr, Vr, 0u)][tid] & 0xFFFFu, (uint32_t)S.pub_right[r][tid - 1u]);
+                on_other(S.list[slot_of(Wr, Vr, 0u)][tid] & 0xFFFFu, idbase + (r << 6) - 1u);   // the site on my left
             }
         }
     };
