@@ -40,16 +40,18 @@ HBM_FALLBACK_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md, used o
 
 # Algorithmic bytes per site per launch.
 BYTES_PER_SITE = {
-    "k_tile_blocks": 1.0 + 0.25 + 4.0 + 0.125 + (16.0 + 1024.0) / 4096.0,  # spins R, bond bits W, labels W, root bitmap W, border + edge records W
+    "k_tile_blocks": 1.0 + 0.25 + 0.25 + 4.0 + 0.125 + (16.0 + 1024.0) / 4096.0,  # spins R, draw masks R, bond bits W, labels W, root bitmap W, border + edge records W
     "k_tile_merge": (16.0 + 1024.0) / 4096.0,                    # border + edge records R (root links touched by the unions come on top)
-    "k_tile_flip": 4.0 + 0.125 + 4.0 + 1.0,                          # labels R, root bitmap R, canonical labels W, spins W
+    "k_tile_flip": 4.0 + 0.125 + 4.0 + 1.0 + 0.25,                   # labels R, root bitmap R, canonical labels W, spins W, next sweep's draw masks W
 }
-BYTES_PER_SITE_LAZY = dict(BYTES_PER_SITE, k_tile_flip=4.0 + 0.125 + 1.0)
+BYTES_PER_SITE_LAZY = dict(BYTES_PER_SITE, k_tile_flip=4.0 + 0.125 + 1.0 + 0.25)
 
-# The tile kernel is bound by instruction issue, not by HBM (profiles/README.md), so it is ALSO reported against an
-# integer-ALU roofline: algorithmic lane-operations per site = 0.5 Philox4x32-10 calls x (20 32x32->64
-# multiplies + 20 three-input XORs) + 2 threshold compares + 2 spin compares; peak = SMs x 128 lanes x SM clock.
-ALU_OPS_PER_SITE = {"k_tile_blocks": 0.5 * 40 + 2 + 2}
+# Every kernel of the sweep is bound by instruction issue rather than by HBM (profiles/README.md), so the whole sweep is
+# ALSO reported against an integer-ALU roofline: algorithmic lane-operations per site = 0.5 Philox4x32-10
+# bond calls x (20 32x32->64 multiplies + 20 three-input XORs) + 2 threshold tests + 2 spin compares, + one Philox call
+# (40) per cluster; peak = SMs x 128 int32 lanes x SM clock.
+ALU_OPS_PER_SITE_BONDS = 0.5 * 40 + 2 + 2
+ALU_OPS_PER_CLUSTER = 40
 B200_SMS, B200_LANES_PER_SM = 148, 128
 
 
@@ -283,15 +285,18 @@ def run_gpu(args):
         roofline = {"kernel": top, "bound": "hbm", "achieved": a, "peak": peak, "unit": "GB/s",
                     "frac": (a / peak) if a else None, "traffic": ncu_traffic(args.workload, top),
                     "peak_source": peak_src,
-                    "algorithmic_bytes_per_launch": bps.get(top, 0) * N}
+                    "algorithmic_bytes_per_launch": bps.get(top, 0) * N,
+                    "limited_by": "instruction issue (integer ALU pipe), not HBM: see profiles/README.md" if top == "k_tile_blocks" else None}
     roofline_alu = None
-    if kernels and roofline and roofline["kernel"] in ALU_OPS_PER_SITE:
+    if kernels and roofline and stats["path"] == 1 and not args.label_equivalence:
         clk = ((clocks or {}).get("sm_mhz") or 1965.0) * 1e6
-        ops = ALU_OPS_PER_SITE[roofline["kernel"]] * N
-        a = ops / (kernels[roofline["kernel"]]["ms_per_launch"] * 1e-3) / 1e12
+        ops = ALU_OPS_PER_SITE_BONDS * N + ALU_OPS_PER_CLUSTER * float(obs.get("n_clusters", 0))
+        a = ops / (elapsed_ms / args.steps * 1e-3) / 1e12
         pk = B200_SMS * B200_LANES_PER_SM * clk / 1e12
-        roofline_alu = {"kernel": roofline["kernel"], "bound": "alu", "achieved": a, "peak": pk, "unit": "Tlane-op/s",
-                        "frac": a / pk, "traffic": roofline["traffic"], "algorithmic_ops_per_launch": ops,
+        tr = [ncu_traffic(args.workload, k) for k in kernels]
+        roofline_alu = {"kernel": "whole sweep (" + " + ".join(kernels) + ")", "bound": "alu", "achieved": a, "peak": pk,
+                        "unit": "Tlane-op/s", "frac": a / pk, "traffic": sum(tr) if all(tr) else None,
+                        "algorithmic_ops_per_sweep": ops,
                         "peak_source": "148 SMs x 128 int32 lanes x SM clock under load (B200_PROFILING.md unit counts)"}
     sweep_bytes = sum(v for v in bps.values()) * N
     sweep_floor_ms = sweep_bytes / (peak * 1e9) * 1e3
@@ -321,10 +326,10 @@ def run_gpu(args):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N, "d2h_bytes_per_step": N, "steps": e2e_steps,
                 "what": "sw_set_state(host spins) + sw_sweep(1) + sw_get_spins(host) per step, pinned host memory"},
         "gpu_launches": launches,
-        # the dominant kernel is bound by its integer ALU pipe (profiles/README.md), so `roofline` is the ALU view and
-        # the HBM view north_star asks for sits beside it (for the whole sweep: sweep_model.frac_of_min_traffic_roofline)
-        "roofline": roofline_alu if roofline_alu else roofline,
-        "roofline_hbm": roofline,
+        # `roofline`: the HBM view north_star asks for, for the dominant kernel (its DRAM traffic equals its algorithmic
+        # bytes; what limits it is instruction issue: profiles/README.md).  `roofline_alu`: the ALU view of the whole sweep.
+        "roofline": roofline,
+        "roofline_alu": roofline_alu,
         "cpu_baseline": cpu_baseline,
         "kernels": kernels,
         "sweep_model": {"bytes_per_site": sum(bps.values()), "floor_ms_at_peak": sweep_floor_ms,
