@@ -217,13 +217,12 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
         const uint32_t lab[4] = {l.x, l.y, l.z, l.w};
         const uint32_t rb = (rq[k] >> (x4 & 12u)) & 15u;
         const uint32_t id0 = ((yk0 + 2 * k) << 6) + x4;
+        // where the chase of a root starts: its own entry.  All four entries are stored with one 16-byte store; the
+        // entries of sites that are not roots are never read (every lookup goes to a root's id).
+        *reinterpret_cast<uint4 *>(&s_root[id0]) = l;
         uint32_t id[4];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const bool isroot = (rb >> j) & 1u;
-            if (isroot) s_root[id0 + j] = lab[j];              // where the chase of this root starts
-            id[j] = isroot ? id0 + j : lab[j];
-        }
+        for (int j = 0; j < 4; ++j) id[j] = ((rb >> j) & 1u) ? id0 + j : lab[j];
         ids[2 * k] = id[0] | (id[1] << 16);
         ids[2 * k + 1] = id[2] | (id[3] << 16);
         work |= rb << (4 * k);
