@@ -161,18 +161,19 @@ int sweep_once(sw_ctx *c, bool count_clusters)
     const Params P = make_params(c, c->t);
     if (c->tiled) {
         const unsigned tiles = (unsigned)(c->N / sw::kTileSites);
+        const dim3 tgrid(c->L / sw::kTile, c->L / sw::kTile);      // one CTA per tile, (tx, ty)
         if (c->draws_t != c->t) {        // first sweep after sw_init / sw_set_state: nobody has made this sweep's bond draws yet
             c->launches += 1;
-            sw::k_draws<<<tiles, 256, 0, c->stream>>>(c->d_draws, P);
+            sw::k_draws<<<tgrid, 256, 0, c->stream>>>(c->d_draws, P);
         }
         { Timed tm(c, SLOT_TILE);
-          sw::k_tile_blocks<<<tiles, sw::kBlkThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_edges, c->d_draws, P); }
+          sw::k_tile_blocks<<<tgrid, sw::kBlkThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_edges, c->d_draws, P); }
         { Timed tm(c, SLOT_MERGE);
           sw::k_tile_merge<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_edges, P, tiles); }
         { Timed tm(c, SLOT_FLIP);
           auto flip = c->lazy ? (count_clusters ? sw::k_tile_flip<false, true, true> : sw::k_tile_flip<false, true, false>)
                               : (count_clusters ? sw::k_tile_flip<true, true, true> : sw::k_tile_flip<true, true, false>);
-          flip<<<tiles, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, c->d_draws); }
+          flip<<<tgrid, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, c->d_draws); }
         c->draws_t = c->t + 1;           // the flip kernel made the draws of the next sweep on the side
         c->labels_flat = !c->lazy;
     } else if (c->label_equiv) {
@@ -225,7 +226,7 @@ int ensure_flat(sw_ctx *c)
     const Params P = make_params(c, c->t);
     c->launches += 1;
     if (c->tiled)       // lazy mode: the forest of the last sweep is still in place (tile-local ids + root links)
-        sw::k_tile_flip<true, false, false><<<(unsigned)(c->N / sw::kTileSites), sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, nullptr);
+        sw::k_tile_flip<true, false, false><<<dim3(c->L / sw::kTile, c->L / sw::kTile), sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, nullptr);
     else
         sw::k_flatten_generic<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_labels, P);
     SW_CUDA(c, cudaGetLastError());

@@ -128,7 +128,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t bx = tid & 7u, by = tid >> 3;
     const uint32_t L = P.L, tiles_x = L >> 6;
-    const uint32_t ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
+    const uint32_t ty = blockIdx.y, tx = blockIdx.x, tile = ty * tiles_x + tx;   // grid = (tiles_x, tiles_x): no division
     const uint32_t X0 = tx << 6, Y0 = ty << 6;
     const uint32_t x0 = X0 + (bx << 3), y0 = Y0 + (by << 2);
     const uint32_t origin = Y0 * L + X0;                       // global index of the tile's first site
@@ -172,7 +172,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
         // The threshold tests of this sweep's draws were made ahead of time (tile_draw_masks in sw_tiled.cuh: by the flip
         // kernel of the previous sweep while it waited for its loads, or by k_draws): bit 8r + c of dm.x / dm.y says
         // whether the right / down draw of my site (r, c) is below the threshold.
-        const uint2 dm = draws[blockIdx.x * kBlkThreads + tid];
+        const uint2 dm = draws[tile * kBlkThreads + tid];
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
             const uint32_t a0 = s[r].x, a1 = s[r].y;
@@ -215,7 +215,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
             TileBorder b;
             b.right_col = (unsigned long long)r_lo | ((unsigned long long)r_hi << 32);
             b.bottom_row = (unsigned long long)b_lo | ((unsigned long long)b_hi << 32);
-            border[blockIdx.x] = b;
+            border[tile] = b;
         }
     }
 
@@ -387,7 +387,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
             uint32_t g[8];
 #pragma unroll
             for (int c = 0; c < 8; ++c) g[c] = ((rootm >> (8 * r + c)) & 1u) ? lab[c] : global_of(lab[c]);
-            uint4 *ep = reinterpret_cast<uint4 *>((r == 0 ? edges[blockIdx.x].top : edges[blockIdx.x].bottom) + 8u * bx);
+            uint4 *ep = reinterpret_cast<uint4 *>((r == 0 ? edges[tile].top : edges[tile].bottom) + 8u * bx);
             ep[0] = make_uint4(g[0], g[1], g[2], g[3]);
             ep[1] = make_uint4(g[4], g[5], g[6], g[7]);
         }
@@ -409,7 +409,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
             const uint32_t v = bx == 0u ? col_l[r] : col_r[r];
             g[r] = ((rootm >> (8 * r + c)) & 1u) ? v : global_of(v);
         }
-        *reinterpret_cast<uint4 *>((bx == 0u ? edges[blockIdx.x].left : edges[blockIdx.x].right) + 4u * by) = make_uint4(g[0], g[1], g[2], g[3]);
+        *reinterpret_cast<uint4 *>((bx == 0u ? edges[tile].left : edges[tile].right) + 4u * by) = make_uint4(g[0], g[1], g[2], g[3]);
     }
 }
 

@@ -86,8 +86,8 @@ __global__ void __launch_bounds__(256)
 k_draws(uint2 *__restrict__ draws, Params P)
 {
     const uint32_t tiles_x = P.L >> 6;
-    const uint32_t ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
-    tile_draw_masks(draws, blockIdx.x, (ty << 6) * P.L + (tx << 6), threadIdx.x, P.t, P);
+    const uint32_t ty = blockIdx.y, tx = blockIdx.x, tile = ty * tiles_x + tx;   // grid = (tiles_x, tiles_x): no division
+    tile_draw_masks(draws, tile, (ty << 6) * P.L + (tx << 6), threadIdx.x, P.t, P);
 }
 
 // ---- kernel 2: merge across tile borders -------------------------------------------------------
@@ -188,7 +188,7 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
     const uint32_t tid = threadIdx.x;
     const uint32_t lane = tid & 31u, warp = tid >> 5;
     const uint32_t L = P.L, tiles_x = L >> 6;
-    const uint32_t ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
+    const uint32_t ty = blockIdx.y, tx = blockIdx.x, tile = ty * tiles_x + tx;   // grid = (tiles_x, tiles_x): no division
     const uint32_t origin = (ty << 6) * L + (tx << 6);
     const uint32_t x4 = (lane & 15u) << 2;                     // my first column inside the tile
     const uint32_t yk0 = warp * kFlipRows + (lane >> 4);       // my tile row for k = 0 (k-th: + 2k)
@@ -210,7 +210,7 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
         rq[k] = rootbits[i0 >> 4];
     }
     // while those loads are on their way: the bond draws of the NEXT sweep for this tile (pure arithmetic, see above)
-    if (kSpins && next_draws) tile_draw_masks(next_draws, blockIdx.x, origin, tid, P.t + 1u, P);
+    if (kSpins && next_draws) tile_draw_masks(next_draws, tile, origin, tid, P.t + 1u, P);
 #pragma unroll
     for (int k = 0; k < kFlipAcc; ++k) {
         const uint4 l = lq[k];
@@ -276,7 +276,7 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
     }
     if (kCount) {
         canon = __reduce_add_sync(0xFFFFFFFFu, canon);
-        if (lane == 0) tile_clusters[blockIdx.x * (kFlipThreads / 32) + warp] = canon;
+        if (lane == 0) tile_clusters[tile * (kFlipThreads / 32) + warp] = canon;
     }
 }
 
