@@ -119,6 +119,17 @@ bool host_threshold(double K, uint64_t *T)
     return true;
 }
 
+// the per-sweep halves of Philox rounds 0 and 1 (philox_sweep in sw_common.cuh)
+void sweep_keys(const Params &P, uint32_t t, uint32_t k[3])
+{
+    const uint64_t m1t = 0xCD9E8D57ull * t;
+    const uint32_t a0 = (uint32_t)(m1t >> 32) ^ P.rk0[0], a1 = (uint32_t)m1t;
+    const uint64_t m0a = 0xD2511F53ull * a0;
+    k[0] = a1 ^ P.rk0[1];
+    k[1] = (uint32_t)(m0a >> 32) ^ P.rk1[1];
+    k[2] = (uint32_t)m0a;
+}
+
 Params make_params(const sw_ctx *c, uint64_t t)
 {
     Params P{};
@@ -133,6 +144,8 @@ Params make_params(const sw_ctx *c, uint64_t t)
     P.log2L = 0xFFFFFFFFu;
     for (uint32_t b = 0; b < 17; ++b) if ((1u << b) == c->L) P.log2L = b;
     P.divL_magic = ((1ull << 40) + c->L - 1) / c->L;
+    sweep_keys(P, P.t, P.pk_t);
+    sweep_keys(P, P.t + 1u, P.pk_n);
     return P;
 }
 

@@ -26,6 +26,8 @@ struct Params {
     uint32_t log2L;       // log2(L) if L is a power of two, else 0xFFFFFFFF
     uint64_t N;           // L * L (up to 2^32)
     uint64_t divL_magic;  // ceil(2^40 / L): (d * magic) >> 40 == d / L for d < 2^24 (L <= 2^16)
+    uint32_t pk_t[3];     // philox_sweep constants of sweep t (see there), and ...
+    uint32_t pk_n[3];     // ... of sweep t + 1 (the flip kernel makes the next sweep's bond draws)
 };
 
 __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -44,12 +46,36 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
     return make_uint4(c0, c1, c2, c3);
 }
 
+// Philox4x32-10 for the draws of a sweep: counter (idx, 0, t, purpose) with idx < 2^32.  Counter words 1 and 2 are the
+// same for every thread, so the halves of rounds 0 and 1 that only depend on them are computed once per sweep on the
+// host (sweep_keys in sw_api.cu): k[0] = lo(M1 t) ^ rk0[1], k[1] = hi(M0 A0) ^ rk1[1], k[2] = lo(M0 A0) with
+// A0 = hi(M1 t) ^ rk0[0].  Bit for bit the same function as philox4x32_10(idx, 0, t, purpose): 37 instead of 40
+// multiply / xor instructions per call.
+__device__ __forceinline__ uint4 philox_sweep(uint32_t idx, uint32_t purpose, const uint32_t (&k)[3], const Params &P)
+{
+    constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+    uint32_t c2 = __umulhi(M0, idx) ^ purpose ^ P.rk1[0], c3 = M0 * idx;             // round 0
+    uint32_t c0 = __umulhi(M1, c2) ^ k[0], c1 = M1 * c2;                             // round 1
+    c2 = c3 ^ k[1];
+    c3 = k[2];
+#pragma unroll
+    for (int r = 2; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
+        const uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+        c0 = hi1 ^ c1 ^ P.rk0[r];
+        c1 = lo1;
+        c2 = hi0 ^ c3 ^ P.rk1[r];
+        c3 = lo0;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
 // floor(w * q / 2^32): the draw -> state map (R9)
 __device__ __forceinline__ uint32_t state_from_draw(uint32_t w, uint32_t q) { return __umulhi(w, q); }
 
 __device__ __forceinline__ uint32_t flip_state(uint32_t root, const Params &P)
 {
-    return state_from_draw(philox4x32_10(root, 0u, P.t, kPurposeFlip, P).x, P.q);
+    return state_from_draw(philox_sweep(root, kPurposeFlip, P.pk_t, P).x, P.q);
 }
 
 // ---- union-find on global memory -------------------------------------------------------------

@@ -59,7 +59,7 @@ __device__ __forceinline__ uint32_t shift_in_not_below(uint32_t mask, uint32_t d
 // 256 threads per tile: thread u makes the draws of rows 2h, 2h + 1 (h = u % 2) of block u / 2: one Philox call per
 // site pair (words: right, down, right, down), last pair first so that the bits are shifted in in order.
 __device__ __forceinline__ void tile_draw_masks(uint2 *__restrict__ draws, uint32_t tile, uint32_t origin, uint32_t u,
-                                                uint32_t t, const Params &P)
+                                                const uint32_t (&pk)[3], const Params &P)
 {
     const uint32_t b = u >> 1, h = u & 1u, bx = b & 7u, by = b >> 3;
     const uint32_t above = ~P.thr_m1;                          // 2^32 - T (T >= 1; T = 0 is masked by thr_any)
@@ -69,7 +69,7 @@ __device__ __forceinline__ void tile_draw_masks(uint2 *__restrict__ draws, uint3
         const uint32_t pair0 = (origin + ((by << 2) + 2u * h + rr) * P.L + (bx << 3)) >> 1;
 #pragma unroll
         for (int p = 3; p >= 0; --p) {
-            const uint4 d = philox4x32_10(pair0 + p, 0u, t, kPurposeBond, P);
+            const uint4 d = philox_sweep(pair0 + p, kPurposeBond, pk, P);
             off_r = shift_in_not_below(off_r, d.z, above);
             off_d = shift_in_not_below(off_d, d.w, above);
             off_r = shift_in_not_below(off_r, d.x, above);
@@ -87,7 +87,7 @@ k_draws(uint2 *__restrict__ draws, Params P)
 {
     const uint32_t tiles_x = P.L >> 6;
     const uint32_t ty = blockIdx.y, tx = blockIdx.x, tile = ty * tiles_x + tx;   // grid = (tiles_x, tiles_x): no division
-    tile_draw_masks(draws, tile, (ty << 6) * P.L + (tx << 6), threadIdx.x, P.t, P);
+    tile_draw_masks(draws, tile, (ty << 6) * P.L + (tx << 6), threadIdx.x, P.pk_t, P);
 }
 
 // ---- kernel 2: merge across tile borders -------------------------------------------------------
@@ -210,7 +210,7 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
         rq[k] = rootbits[i0 >> 4];
     }
     // while those loads are on their way: the bond draws of the NEXT sweep for this tile (pure arithmetic, see above)
-    if (kSpins && next_draws) tile_draw_masks(next_draws, tile, origin, tid, P.t + 1u, P);
+    if (kSpins && next_draws) tile_draw_masks(next_draws, tile, origin, tid, P.pk_n, P);
 #pragma unroll
     for (int k = 0; k < kFlipAcc; ++k) {
         const uint4 l = lq[k];
