@@ -125,6 +125,31 @@ def test_label_equivalence_round_count_near_the_papers():
     assert 5.0 <= mean_rounds <= 14.0
 
 
+def test_many_sweeps_per_call_and_state_changes_in_between():
+    # sw_sweep(n) makes the bond draws of sweep t + 1 while sweep t runs and counts clusters only in the last sweep of
+    # a call: the result must not depend on how the sweeps are grouped into calls, nor on sw_set_state / sw_init in between
+    L, q, K = 192, 3, wl.k_critical(3)
+    gpu, cpu = SwendsenWang(L, q, K, 21), Oracle(L, q, K, 21)
+    gpu.init("random"); cpu.init("random")
+    gpu.sweep(7); cpu.sweep(7)
+    compare_after_sweep(gpu, cpu, "(7 sweeps in one call)")
+    gpu.sweep(1); gpu.sweep(3); cpu.sweep(4)
+    compare_after_sweep(gpu, cpu, "(1 + 3 sweeps)")
+    spins = wl.spins_uniform_random(L, q, 5)
+    gpu.set_state(spins, 3); cpu.set_state(spins, 3)          # an earlier sweep counter: the draws made ahead are stale
+    gpu.sweep(2); cpu.sweep(2)
+    compare_after_sweep(gpu, cpu, "(after sw_set_state to t = 3)")
+    gpu.set_state(spins, 5); cpu.set_state(spins, 5)          # the counter the draws were made for, other spins
+    gpu.sweep(1); cpu.sweep(1)
+    compare_after_sweep(gpu, cpu, "(after sw_set_state to the current t)")
+    gpu.init("ordered"); cpu.init("ordered")
+    gpu.sweep(2); cpu.sweep(2)
+    compare_after_sweep(gpu, cpu, "(after sw_init)")
+    rows_g, rows_c = gpu.sweep_measure(3), cpu.sweep_measure(3)
+    assert np.array_equal(rows_g, rows_c)
+    compare_after_sweep(gpu, cpu, "(after sw_sweep_measure)")
+
+
 def test_tiled_path_is_selected_and_counts_kernels():
     g = SwendsenWang(128, 2, 0.5, 1)
     g.init("ordered")
