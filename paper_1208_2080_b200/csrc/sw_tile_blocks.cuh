@@ -173,14 +173,24 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
         // kernel of the previous sweep while it waited for its loads, or by k_draws): bit 8r + c of dm.x / dm.y says
         // whether the right / down draw of my site (r, c) is below the threshold.
         const uint2 dm = draws[tile * kBlkThreads + tid];
+        if (P.q == 2u) {                                       // spins are 0 / 1: "equal" is bit 0 of the XNOR (pack4 looks at bit 0 only)
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const uint32_t a0 = s[r].x, a1 = s[r].y;
-            const uint32_t n0 = __funnelshift_r(a0, a1, 8), n1 = __funnelshift_r(a1, nx >> (8 * r), 8);
-            const uint32_t eq_r = pack4(__vcmpeq4(a0, n0)) | (pack4(__vcmpeq4(a1, n1)) << 4);
-            const uint32_t eq_d = pack4(__vcmpeq4(a0, s[r + 1].x)) | (pack4(__vcmpeq4(a1, s[r + 1].y)) << 4);
-            R |= eq_r << (8 * r);
-            D |= eq_d << (8 * r);
+            for (int r = 0; r < 4; ++r) {
+                const uint32_t a0 = s[r].x, a1 = s[r].y;
+                const uint32_t n0 = __funnelshift_r(a0, a1, 8), n1 = __funnelshift_r(a1, nx >> (8 * r), 8);
+                R |= (pack4(~(a0 ^ n0)) | (pack4(~(a1 ^ n1)) << 4)) << (8 * r);
+                D |= (pack4(~(a0 ^ s[r + 1].x)) | (pack4(~(a1 ^ s[r + 1].y)) << 4)) << (8 * r);
+            }
+        } else {
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const uint32_t a0 = s[r].x, a1 = s[r].y;
+                const uint32_t n0 = __funnelshift_r(a0, a1, 8), n1 = __funnelshift_r(a1, nx >> (8 * r), 8);
+                const uint32_t eq_r = pack4(__vcmpeq4(a0, n0)) | (pack4(__vcmpeq4(a1, n1)) << 4);
+                const uint32_t eq_d = pack4(__vcmpeq4(a0, s[r + 1].x)) | (pack4(__vcmpeq4(a1, s[r + 1].y)) << 4);
+                R |= eq_r << (8 * r);
+                D |= eq_d << (8 * r);
+            }
         }
         R &= dm.x;
         D &= dm.y;
