@@ -51,8 +51,8 @@ __device__ __forceinline__ uint32_t pack4(uint32_t eq) { return ((eq & 0x0101010
 // mask * 2 + (draw >= T): add.cc sets the carry iff draw + (2^32 - T) overflows, addc shifts it into the mask
 __device__ __forceinline__ uint32_t shift_in_not_below(uint32_t mask, uint32_t draw, uint32_t above)
 {
-    uint32_t t, out;
-    asm("add.cc.u32 %0, %2, %3;\n\taddc.u32 %1, %4, %4;" : "=r"(t), "=r"(out) : "r"(draw), "r"(above), "r"(mask));
+    uint32_t out;
+    asm("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\taddc.u32 %0, %3, %3;\n\t}" : "=r"(out) : "r"(draw), "r"(above), "r"(mask));
     return out;
 }
 
