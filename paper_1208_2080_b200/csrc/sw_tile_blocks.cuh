@@ -2,9 +2,10 @@
 //
 //   k_tile_blocks   step (1) + the tile-local part of step (2) of the sweep ("the
 //                   calculation [is] done independently on each site"; :42 "proper label" = the
-//                   smallest site of the cluster).  Same inputs and outputs as a tile kernel must
-//                   have for k_tile_merge / k_tile_flip (sw_tiled.cuh): bonds, labels = global index
-//                   of the tile-local root, root bitmap, border record, column labels.
+//                   smallest site of the cluster).  In: spins, and the "draw < T" bits of this sweep's
+//                   bonds (made one sweep ahead, sw_tiled.cuh).  Out, for k_tile_merge / k_tile_flip:
+//                   bonds, labels (tile-local roots: their own global index; other sites: the 12-bit
+//                   tile-local id of their root), root bitmap, border record, edge record.
 //
 // A tile is 64 x 64 sites, a CTA of 128 threads owns it; thread (bx = tid % 8, by = tid / 8) owns the
 // block of 8 columns x 4 rows at (8 bx, 4 by): its 32 sites are the 32 bits of one register (bit
@@ -17,7 +18,7 @@
 //   * "which component is site j in" is kept bit-sliced in five plane registers.
 // Only the components of the blocks (about 0.2 per site at q = 2, K_c instead of 0.53 horizontal
 // runs per site) go through the shared-memory union-find, over the bonds that cross a block edge
-// (0.19 per site): first up-link of every component by plain store, the rest with atomicMin.
+// (0.16 per site): first up-link of every component by plain store, the rest with an atomic minimum.
 #pragma once
 
 #include "sw_common.cuh"
@@ -33,7 +34,7 @@ constexpr uint32_t kDecodeMul = (1u << 24) | (1u << 17) | (1u << 10) | (1u << 3)
 struct BlkShared {
     uint16_t parent[kTileSites];              // union-find over tile-local site ids (y * 64 + x): component seeds are linked; a site of
                                               // the right column of a block points at its seed (the block on its right links to the site)
-    uint32_t list[kBlkSlots][kBlkThreads];    // per thread, slot k: component mask -> seed id | seed bit << 16 -> global label of its root
+    uint32_t list[kBlkSlots][kBlkThreads];    // per thread, slot k: component mask -> seed id | seed bit << 16 -> tile-local id of its root
     uint16_t pub_bottom[8][kBlkThreads];      // seed id of the component of my bottom-row site c
     uint32_t edge[kBlkThreads];               // what the blocks below / to the right need to know about a block: bits 0-7 down
                                               // bonds of row 3, 8-15 right bonds of row 3, 16-19 right bonds of column 7,
@@ -46,7 +47,7 @@ constexpr int kBlkBufSlot = 14;
 static_assert((kBlkSlots - kBlkBufSlot) * kBlkThreads >= (kBlkThreads / 32) * kBlkExtraCap, "link buffer too small");
 
 // ---- union-find on 16-bit parents ------------------------------------------------------------------
-// Same rules as unite_s (sw_tiled.cuh): links point to smaller ids, plain stores only ever replace a link
+// Links point to smaller ids, plain stores only ever replace a link
 // by a link to an ancestor, hooks are an atomic minimum (here a CAS on the 32-bit word that holds the entry:
 // a plain 16-bit store to either half in between makes the CAS fail and retry).
 __device__ __forceinline__ uint32_t atomic_min_u16(uint16_t *base, uint32_t idx, uint32_t val)
