@@ -150,6 +150,36 @@ def test_many_sweeps_per_call_and_state_changes_in_between():
     compare_after_sweep(gpu, cpu, "(after sw_sweep_measure)")
 
 
+def test_randomised_configurations():
+    # 40 seeded random (L, q, K, seed, flags, start / crafted state, sweep counter, sweeps per call) combinations
+    import random
+    rng = random.Random(12345)
+    for case in range(40):
+        L = rng.choice([64, 128, 192, 256, 320])
+        q = rng.choice([2, 2, 3, 4, 5, 10, 37, 255])
+        K = rng.choice([0.0, math.inf, wl.k_critical(q), 0.3, 1.5, 3.0, wl.k_critical(q) * 1.05, 1e-6, 30.0])
+        seed, flags = rng.getrandbits(64), rng.choice([0, 0, sw.FLAG_LAZY_LABELS])
+        t0 = rng.choice([0, 1, 7, 0xFFFFFFF0])
+        gpu, cpu = SwendsenWang(L, q, K, seed, flags=flags), Oracle(L, q, K, seed)
+        if rng.random() < 0.5:
+            if rng.random() < 0.7:
+                spins = wl.spins_uniform_random(L, q, rng.getrandbits(31))
+            else:
+                spins = wl.spins_dominoes(L, rng.randint(0, 1), rng.randint(0, 1), rng.random() < 0.5, q=min(q, 251))
+            gpu.set_state(spins, t0); cpu.set_state(spins, t0)
+        else:
+            start = rng.choice(["random", "ordered"])
+            gpu.init(start); cpu.init(start)
+        n = rng.choice([1, 2, 3])
+        gpu.sweep(n); cpu.sweep(n)
+        what = f"(case {case}: L={L} q={q} K={K} flags={flags} n={n})"
+        assert gpu.measure() == cpu.measure(), what                 # (before any label read-back: lazy mode)
+        compare_after_sweep(gpu, cpu, what)
+        gpu.sweep(1); cpu.sweep(1)
+        compare_after_sweep(gpu, cpu, what + " + 1")
+        gpu.close(); cpu.close()
+
+
 def test_tiled_path_is_selected_and_counts_kernels():
     g = SwendsenWang(128, 2, 0.5, 1)
     g.init("ordered")
