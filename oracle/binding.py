@@ -4,6 +4,7 @@ Argument marshalling only; every number comes from sw_oracle.cpp.
 """
 import ctypes as C
 import math
+import os
 
 import numpy as np
 
@@ -24,7 +25,8 @@ class OracleError(RuntimeError):
 def lib():
     global _lib
     if _lib is None:
-        l = C.CDLL(_build.build())
+        # SWO_LIB: tests/oracle_mutations.py points the binding at a deliberately broken copy of the oracle
+        l = C.CDLL(os.environ.get("SWO_LIB") or _build.build())
         u8p, u32p, u64p = C.POINTER(C.c_uint8), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)
         vp = C.c_void_p
         l.swo_philox4x32_10.argtypes = [u32p, u32p, u32p]; l.swo_philox4x32_10.restype = None

@@ -191,3 +191,58 @@ def test_comparison_is_strict_draw_below_threshold(golden):
         sim.init("ordered")
         sim.sweep(1)
         assert sim.get_bonds()[1] & 2 == want
+
+
+@pytest.mark.parametrize("L,q,K,start", [(12, 2, wl.k_critical(2), "random"), (20, 3, 0.9, "random"), (9, 5, 1.3, "ordered")])
+def test_sweep_measure_rows_follow_the_header_column_order(L, q, K, start):
+    # swo_sweep_measure(n) must equal n x (swo_sweep(1), swo_measure) with the columns of oracle/sw_oracle.h:
+    # [energy_bonds, n_clusters, largest_cluster, mag_counts[0..q-1]].  n_clusters and largest_cluster are NOT taken
+    # from the oracle's counters here: they are recounted by scipy from the bonds of a second, step-by-step run of the
+    # same chain, so a swap of the two columns (or of &row[1] / &row[2]) fails.
+    n, seed = 12, 17
+    series = Oracle(L, q, K, seed)
+    series.init(start)
+    rows = series.sweep_measure(n)
+    assert rows.shape == (n, 3 + q) and rows.dtype == np.uint64
+    step = Oracle(L, q, K, seed)
+    step.init(start)
+    saw_different = False
+    for k in range(n):
+        step.sweep(1)
+        spins = step.get_spins().reshape(L, L)
+        _, nc, big = canonical_by_scipy(step.get_bonds().reshape(L, L))
+        want = [energy_bonds_numpy(spins), nc, big] + np.bincount(spins.reshape(-1), minlength=q).tolist()
+        assert rows[k].tolist() == want, f"row {k}"
+        saw_different |= nc != big
+    assert saw_different                                   # otherwise a swap of columns 1 and 2 could hide
+    assert np.array_equal(series.get_spins(), step.get_spins()) and series.get_time() == step.get_time() == n
+
+
+def test_init_and_set_state_reset_the_chain():
+    # sw_init sets t = 0 and forgets the labels: a chain re-initialised after some sweeps repeats the fresh chain exactly
+    # (the sweep counter is a word of every Philox counter, so a stale t would change every draw)
+    L, q, K, seed = 10, 3, 1.0, 5
+    fresh = Oracle(L, q, K, seed)
+    fresh.init("random")
+    fresh.sweep(3)
+    again = Oracle(L, q, K, seed)
+    again.init("ordered")
+    again.sweep(2)
+    again.init("random")
+    assert again.get_time() == 0
+    m = again.measure()
+    assert m["n_clusters"] == 0 and m["largest_cluster"] == 0
+    with pytest.raises(orc.OracleError):
+        again.get_labels()
+    again.sweep(3)
+    assert again.get_time() == 3
+    assert np.array_equal(again.get_spins(), fresh.get_spins()) and np.array_equal(again.get_labels(), fresh.get_labels())
+    # set_state(spins, t) resumes at exactly that t
+    mid = Oracle(L, q, K, seed)
+    mid.init("random")
+    mid.sweep(1)
+    resumed = Oracle(L, q, K, seed)
+    resumed.set_state(mid.get_spins(), 1)
+    assert resumed.get_time() == 1
+    resumed.sweep(2)
+    assert np.array_equal(resumed.get_spins(), fresh.get_spins())
