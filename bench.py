@@ -6,12 +6,15 @@
 A step is ONE full sweep (bond activation, tile-local labeling, border merge, flatten to canonical
 labels, flip: SURVEY.md sec. 8(a) rows a1-a5) of the headline workload of BASELINE.json: q = 2 Potts at
 K_c on the 65536 x 65536 periodic lattice (2^32 sites), random start, Philox seed 1.  W untimed sweeps,
-then exactly K sweeps timed with CUDA events on the stream the kernels run on.  The 21 GiB working
-set is far larger than the 126 MB L2, so no L2 flush is needed between sweeps.
+then exactly K sweeps timed with CUDA events on the stream the kernels run on.  The 23.5 GiB working
+set is far larger than the 126 MB L2, so no L2 flush is needed between sweeps.  The per-kernel split and
+the per-sweep time series come from a SECOND pass of K sweeps (events around every kernel), outside the
+headline region.
 
 N > 1: the path does not shard without collectives ("replicas only"), so every
 rank runs an independent replica (seed 1 + rank) and the value is the aggregate of all replicas
-over the slowest rank's time.
+over the slowest rank's time.  `--gpus N` without a torchrun environment starts the N ranks itself
+(re-exec under `python -m torch.distributed.run`); under torchrun WORLD_SIZE must equal N.
 
 --impl reference times the CPU oracle (oracle/, plain single-threaded C++) on the host cores on a
 bounded sample of the same workload; it is a deliberately slow reference program, not a target.
@@ -21,6 +24,7 @@ from __future__ import annotations
 import argparse
 import json
 import os
+import socket
 import statistics
 import subprocess
 import sys
@@ -38,25 +42,47 @@ UNIT = "flips/ns"
 PAPER_FLIPS_PER_NS = 37.30        # PAPER.md:103 (Table 1): L = 65536, q = 2, T_c, 256 x Tesla M2050
 HBM_FALLBACK_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 
-# Algorithmic bytes per site per launch.
-BYTES_PER_SITE = {
-    "k_tile_blocks": 1.0 + 0.25 + 0.25 + 4.0 + 0.125 + (16.0 + 1024.0) / 4096.0,  # spins R, draw masks R, bond bits W, labels W, root bitmap W, border + edge records W
-    "k_tile_merge": (16.0 + 1024.0) / 4096.0,                    # border + edge records R (root links touched by the unions come on top)
-    "k_tile_flip": 4.0 + 0.125 + 4.0 + 1.0 + 0.25,                   # labels R, root bitmap R, canonical labels W, spins W, next sweep's draw masks W
+# Algorithmic bytes per site per launch: what the METHOD must move.
+ALGORITHMIC_BYTES_PER_SITE = {
+    "k_tile_blocks": 1.0 + 0.25 + 4.0,          # a1 + a2: spins R, bond bits W, labels W
+    "k_tile_merge": 24.0 / 64.0,                # a3: 2/T_tile border bonds per site x (two 4-byte finds + one 4-byte atomic), T_tile = 64
+    "k_tile_flip": 4.0 + 4.0 + 1.0,             # a4 + a5: labels R, canonical labels W, spins W
 }
-BYTES_PER_SITE_LAZY = dict(BYTES_PER_SITE, k_tile_flip=4.0 + 0.125 + 1.0 + 0.25)
+# What THIS design moves on top of that (its own auxiliary arrays), reported separately.
+OVERHEAD_BYTES_PER_SITE = {
+    "k_tile_blocks": 0.25 + 0.125 + (16.0 + 1024.0) / 4096.0,   # draw masks R, root bitmap W, border + edge records W
+    "k_tile_merge": (16.0 + 1024.0) / 4096.0 - 24.0 / 64.0 + 1.25,   # records R instead of label reads, + 64-byte DRAM bursts per root link (measured)
+    "k_tile_flip": 0.125 + 0.25,                # root bitmap R, next sweep's draw masks W
+}
+LAZY_SAVES = 4.0                                # SW_FLAG_LAZY_LABELS: no canonical-label write in k_tile_flip
 
-# Every kernel of the sweep is bound by instruction issue rather than by HBM (profiles/README.md), so the whole sweep is
-# ALSO reported against an integer-ALU roofline: algorithmic lane-operations per site = 0.5 Philox4x32-10
-# bond calls x (20 32x32->64 multiplies + 20 three-input XORs) + 2 threshold tests + 2 spin compares, + one Philox call
-# (40) per cluster; peak = SMs x 128 int32 lanes x SM clock.
+# Integer-ALU view of the whole sweep: algorithmic lane-operations per site = 0.5 Philox4x32-10 bond
+# calls x (20 32x32->64 multiplies + 20 three-input XORs) + 2 threshold tests + 2 spin compares, + one Philox call (40)
+# per cluster; peak = SMs x 128 int32 lanes x SM clock.
 ALU_OPS_PER_SITE_BONDS = 0.5 * 40 + 2 + 2
 ALU_OPS_PER_CLUSTER = 40
 B200_SMS, B200_LANES_PER_SM = 148, 128
 
+# the other BASELINE.json configs, measured briefly in the same run: (name, warm-up sweeps, timed sweeps, observables the
+# config asks for every sweep -- None = update only)
+OTHER_CONFIGS = [
+    ("c1_L256_q2", 20, 200, "all"),
+    ("c2_L4096_q2", 40, 40, None),
+    ("c3_L8192_q3", 30, 20, "energy+mag"),
+    ("c3_L8192_q4", 30, 20, "energy+mag"),
+    ("c4_L16384_q10_above", 30, 20, "clusters+largest"),
+    ("c4_L16384_q10_below", 30, 20, "clusters+largest"),
+]
+
 
 def rank_info():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
 
 
 class ClockSampler:
@@ -126,18 +152,18 @@ def ncu_traffic(workload, kernel):
         return None
 
 
-def time_oracle(L, q, K, seed, start, warm, sweeps):
-    from oracle.binding import Oracle
-    sim = Oracle(L, q, K, seed)
-    sim.init(start)
-    if warm:
-        sim.sweep(warm)
-    t0 = time.perf_counter()
-    sim.sweep(sweeps)
-    dt = time.perf_counter() - t0
-    sim.close()
-    return dt
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
+
+# ------------------------------------------------------------------------------------------------ reference arm
 
 def run_reference(args):
     """--impl reference: the oracle as it stands, one thread, on a bounded sample of the workload."""
@@ -162,17 +188,94 @@ def run_reference(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
         "config": {"workload": args.workload, "L": c["L"], "q": c["q"], "K": c["K"], "start": c["start"], "seed": c["seed"],
                    "sample_L": L},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                         "nproc": os.cpu_count(), "cpu_model": cpu_model()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
     return 0
 
 
+# ------------------------------------------------------------------------------------------------ CPU baseline leg
+
+def time_cpu_baseline(args, equilibrated):
+    """The oracle as it stands on this box's host cores, one thread.  `equilibrated` maps a lattice
+    size to (spins, t, q, K, seed) taken from the GPU after its warm-up, so the oracle is timed on a steady-state lattice."""
+    from oracle.binding import Oracle
+    out = {}
+    # headline sample: >= 20 sweeps at L = 4096, q = 2, K_c, from an equilibrated state
+    spins, t, q, K, seed = equilibrated[4096]
+    sim = Oracle(4096, q, K, seed)
+    sim.set_state(spins, t)
+    t0 = time.perf_counter()
+    sim.sweep(args.cpu_baseline_sweeps)
+    dt = time.perf_counter() - t0
+    sim.close()
+    out["L4096"] = {"flips_per_ns": 4096 * 4096 * args.cpu_baseline_sweeps / dt / 1e9, "ns_per_site_sweep": dt * 1e9 / (4096 * 4096 * args.cpu_baseline_sweeps),
+                    "sweeps": args.cpu_baseline_sweeps, "seconds": dt}
+    # config 1: all 200 sweeps from its own random start
+    c1 = wl.CONFIGS["c1_L256_q2"]
+    sim = Oracle(c1["L"], c1["q"], c1["K"], c1["seed"])
+    sim.init(c1["start"])
+    t0 = time.perf_counter()
+    sim.sweep(c1["sweeps"])
+    dt1 = time.perf_counter() - t0
+    sim.close()
+    out["c1_L256"] = {"flips_per_ns": c1["L"] ** 2 * c1["sweeps"] / dt1 / 1e9, "ns_per_site_sweep": dt1 * 1e9 / (c1["L"] ** 2 * c1["sweeps"]),
+                      "sweeps": c1["sweeps"], "seconds": dt1}
+    # one sweep at L = 8192 (q = 3, K_c), equilibrated state
+    if 8192 in equilibrated:
+        spins, t, q, K, seed = equilibrated[8192]
+        sim = Oracle(8192, q, K, seed)
+        sim.set_state(spins, t)
+        t0 = time.perf_counter()
+        sim.sweep(1)
+        dt2 = time.perf_counter() - t0
+        sim.close()
+        out["L8192_q3"] = {"flips_per_ns": 8192 * 8192 / dt2 / 1e9, "ns_per_site_sweep": dt2 * 1e9 / (8192 * 8192), "sweeps": 1, "seconds": dt2}
+    total = sum(v["seconds"] for v in out.values())
+    return {"value": out["L4096"]["flips_per_ns"], "unit": UNIT, "cores": 1, "kind": "oracle",
+            "nproc": os.cpu_count(), "cpu_model": cpu_model(),
+            "sample": f"{args.cpu_baseline_sweeps} sweeps of an equilibrated L=4096 lattice (q=2, K_c: the headline physics; state taken from the GPU "
+                      f"after its warm-up and loaded with swo_set_state), single thread; also config 1 (L=256, all 200 sweeps) and one sweep "
+                      f"at L=8192 (q=3): {total:.1f} s of CPU in all",
+            "samples": out}
+
+
+# ------------------------------------------------------------------------------------------------ GPU arm
+
+def measure_config(name, warm, steps, what, torch, SwendsenWang, sw):
+    """Brief measurement of one of the other BASELINE.json configs: update-only, and with the observables it asks for."""
+    c = wl.CONFIGS[name]
+    L, N = c["L"], c["L"] ** 2
+    sim = SwendsenWang(L, c["q"], c["K"], c["seed"])
+    sim.init(c["start"])
+    sim.sweep(warm)
+    sim.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); sim.sweep(steps); e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    rec = {"L": L, "q": c["q"], "start": c["start"], "warmup": warm, "steps": steps,
+           "flips_per_ns": N / (ms * 1e-3) / 1e9, "ms_per_sweep": ms, "path": sim.stats()["path_name"]}
+    if what:
+        mask = {"all": sw.OBS_ALL, "energy+mag": sw.OBS_ENERGY | sw.OBS_MAG, "clusters+largest": sw.OBS_CLUSTERS | sw.OBS_LARGEST}[what]
+        sim.sweep_measure(2, mask)                                  # warm (first call allocates / sizes scratch)
+        m_steps = min(steps, 50)
+        e0.record(); rows = sim.sweep_measure(m_steps, mask); e1.record()
+        torch.cuda.synchronize()
+        ms_m = e0.elapsed_time(e1) / m_steps
+        rec.update({"observables_every_sweep": what, "flips_per_ns_with_measurement": N / (ms_m * 1e-3) / 1e9,
+                    "ms_per_sweep_with_measurement": ms_m, "last_row": [int(v) for v in rows[-1]]})
+    sim.close()
+    return rec
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
 
+    from paper_1208_2080_b200 import binding as sw
     from paper_1208_2080_b200 import replicas
     from paper_1208_2080_b200.binding import FLAG_DEFAULT, FLAG_LABEL_EQUIVALENCE, FLAG_LAZY_LABELS, SwendsenWang
 
@@ -200,22 +303,18 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- timed region: exactly K sweeps, CUDA events on the stream the kernels are enqueued on
+    # ---- timed region: exactly K sweeps, CUDA events on the stream the kernels are enqueued on; nothing else in it
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
         time.sleep(0.25)
     launches0 = sim.stats()["kernel_launches"]
-    per_kernel_in_region = N >= (1 << 24)          # event overhead (~us per kernel) is negligible only for big lattices
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     wall0 = time.time()
-    if per_kernel_in_region:
-        sim.profile_begin()
     ev0.record()
     sim.sweep(args.steps)
     ev1.record()
-    prof = sim.profile_end() if per_kernel_in_region else None
     barrier()
     wall1 = time.time()
     elapsed_ms = ev0.elapsed_time(ev1)
@@ -226,10 +325,11 @@ def run_gpu(args):
     elapsed_ms = elapsed_s * 1e3
     value = rate / 1e9
 
-    if not per_kernel_in_region:                   # small lattice: separate pass for the per-kernel split
-        sim.profile_begin()
-        sim.sweep(args.steps)
-        prof = sim.profile_end()
+    # ---- second pass, outside the headline region: events around every kernel -> per-kernel split and per-sweep series
+    sim.profile_begin()
+    sim.sweep(args.steps)
+    prof = sim.profile_end()
+    series = sim.last_series
 
     # ---- update + measurement (the paper's second column): sweep + all observables each step
     m_steps = max(1, min(args.steps, 10))
@@ -258,6 +358,7 @@ def run_gpu(args):
     barrier()
     e2e_s = time.perf_counter() - w0
     e2e_value = replicas.aggregate_throughput(N * e2e_steps, e2e_s, device="cuda")[2] / 1e9
+    del host
 
     stats = sim.stats()
     if rank != 0:
@@ -265,30 +366,37 @@ def run_gpu(args):
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline of the dominant kernel
+    # ---- roofline of the dominant kernel: SURVEY.md sec. 8(d) algorithmic bytes over its CUDA-event duration
     peak, peak_src = hbm_peak()
-    bps = BYTES_PER_SITE_LAZY if args.lazy else BYTES_PER_SITE
+    alg = dict(ALGORITHMIC_BYTES_PER_SITE)
+    if args.lazy:
+        alg["k_tile_flip"] -= LAZY_SAVES
     kernels = {}
     for name, rec in (prof or {}).items():
         avg_ms = rec["ms"] / rec["launches"]
-        b = bps.get(name)
-        kernels[name] = {"ms_per_launch": avg_ms, "share": None,
-                         "algorithmic_bytes_per_site": b,
+        b = alg.get(name)
+        kernels[name] = {"ms_per_launch": avg_ms, "launches_per_sweep": rec["launches"] / args.steps, "share": None,
+                         "algorithmic_bytes_per_site": b, "overhead_bytes_per_site": OVERHEAD_BYTES_PER_SITE.get(name),
                          "achieved_gbs": (b * N / (avg_ms * 1e-3) / 1e9) if b else None}
-    tot = sum(k["ms_per_launch"] for k in kernels.values()) or 1.0
+    tot = sum(k["ms_per_launch"] * k["launches_per_sweep"] for k in kernels.values()) or 1.0
     for k in kernels.values():
-        k["share"] = k["ms_per_launch"] / tot
+        k["share"] = k["ms_per_launch"] * k["launches_per_sweep"] / tot
     roofline = None
-    if kernels:
+    tiled = stats["path"] == 1 and not args.label_equivalence
+    if kernels and tiled:
         top = max(kernels, key=lambda n: kernels[n]["ms_per_launch"])
         a = kernels[top]["achieved_gbs"]
         roofline = {"kernel": top, "bound": "hbm", "achieved": a, "peak": peak, "unit": "GB/s",
                     "frac": (a / peak) if a else None, "traffic": ncu_traffic(args.workload, top),
                     "peak_source": peak_src,
-                    "algorithmic_bytes_per_launch": bps.get(top, 0) * N,
-                    "limited_by": "instruction issue (integer ALU pipe), not HBM: see profiles/README.md" if top == "k_tile_blocks" else None}
+                    "algorithmic_bytes_per_launch": alg.get(top, 0) * N,
+                    "algorithmic_bytes_per_site": alg.get(top),
+                    "overhead_bytes_per_site": OVERHEAD_BYTES_PER_SITE.get(top),
+                    "bytes_source": "SURVEY.md sec. 8(d): spins R 1 + bond bits W 0.25 + labels W 4 (a1+a2); labels R 4 + W 4 + spins W 1 (a4+a5); "
+                                    "the design's auxiliary arrays are the separate overhead_bytes_per_site",
+                    "limited_by": "integer ALU pipe (instruction issue), not HBM: see profiles/README.md"}
     roofline_alu = None
-    if kernels and roofline and stats["path"] == 1 and not args.label_equivalence:
+    if kernels and roofline:
         clk = ((clocks or {}).get("sm_mhz") or 1965.0) * 1e6
         ops = ALU_OPS_PER_SITE_BONDS * N + ALU_OPS_PER_CLUSTER * float(obs.get("n_clusters", 0))
         a = ops / (elapsed_ms / args.steps * 1e-3) / 1e12
@@ -298,19 +406,38 @@ def run_gpu(args):
                         "unit": "Tlane-op/s", "frac": a / pk, "traffic": sum(tr) if all(tr) else None,
                         "algorithmic_ops_per_sweep": ops,
                         "peak_source": "148 SMs x 128 int32 lanes x SM clock under load (B200_PROFILING.md unit counts)"}
-    sweep_bytes = sum(v for v in bps.values()) * N
-    sweep_floor_ms = sweep_bytes / (peak * 1e9) * 1e3
+    sweep_alg = sum(alg.values())
+    sweep_floor_ms = sweep_alg * N / (peak * 1e9) * 1e3
     per_gpu_ms = elapsed_ms / args.steps
+    half = series[len(series) // 2:] if series else []
+    time_series = {"ms_per_sweep": [round(v, 4) for v in series], "second_half_mean_ms": (sum(half) / len(half)) if half else None,
+                   "second_half_flips_per_ns": (N / (sum(half) / len(half) * 1e-3) / 1e9) if half else None,
+                   "what": "device time of each sweep of the second (profiled) pass, first kernel start to last kernel end; sweeps "
+                           f"{args.warmup + args.steps} .. {args.warmup + 2 * args.steps - 1} since the start"}
 
-    # ---- the oracle on this box's host cores (reported baseline, rank 0, N = 1 only)
+    # ---- the other BASELINE.json configs, briefly (each closes its context before the next)
+    other = None
+    equilibrated = {}
+    if world == 1 and args.workload == wl.HEADLINE and not args.no_other_configs:
+        sim.close()
+        torch.cuda.empty_cache()
+        other = {}
+        for name, warm, steps, what in OTHER_CONFIGS:
+            try:
+                other[name] = measure_config(name, warm, steps, what, torch, SwendsenWang, sw)
+            except Exception as e:                                   # a failed side measurement must not lose the headline line
+                other[name] = {"error": repr(e)}
+
+    # ---- the oracle on this box's host cores (reported baseline, rank 0, N = 1 only), on equilibrated lattices
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
-        Lc = min(L, args.cpu_baseline_L)
-        dt = time_oracle(Lc, q, K, c["seed"], c["start"], 1, args.cpu_baseline_sweeps)
-        cpu_baseline = {"value": Lc * Lc * args.cpu_baseline_sweeps / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
-                        "host_cores_available": os.cpu_count(),
-                        "sample": f"{args.cpu_baseline_sweeps} sweeps of an L={Lc} lattice (q={q}, K=K_c, {c['start']} start, seed {c['seed']}) "
-                                  f"after 1 warm-up sweep, single thread, {dt:.1f} s"}
+        for Lc, qc, warm in ((4096, 2, 100), (8192, 3, 60)):
+            g = SwendsenWang(Lc, qc, wl.k_critical(qc), 1)
+            g.init("random")
+            g.sweep(warm)
+            equilibrated[Lc] = (g.get_spins(), g.get_time(), qc, wl.k_critical(qc), 1)
+            g.close()
+        cpu_baseline = time_cpu_baseline(args, equilibrated)
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -326,16 +453,17 @@ def run_gpu(args):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N, "d2h_bytes_per_step": N, "steps": e2e_steps,
                 "what": "sw_set_state(host spins) + sw_sweep(1) + sw_get_spins(host) per step, pinned host memory"},
         "gpu_launches": launches,
-        # `roofline`: the HBM view north_star asks for, for the dominant kernel (its DRAM traffic equals its algorithmic
-        # bytes; what limits it is instruction issue: profiles/README.md).  `roofline_alu`: the ALU view of the whole sweep.
         "roofline": roofline,
         "roofline_alu": roofline_alu,
         "cpu_baseline": cpu_baseline,
         "kernels": kernels,
-        "sweep_model": {"bytes_per_site": sum(bps.values()), "floor_ms_at_peak": sweep_floor_ms,
-                        "frac_of_min_traffic_roofline": sweep_floor_ms / per_gpu_ms},
+        "sweep_model": {"algorithmic_bytes_per_site": sweep_alg, "overhead_bytes_per_site": sum(OVERHEAD_BYTES_PER_SITE.values()) if tiled else None,
+                        "floor_ms_at_peak": sweep_floor_ms, "frac_of_min_traffic_roofline": sweep_floor_ms / per_gpu_ms,
+                        "what": "SURVEY.md sec. 8(d): 14.5 + 24/T_tile bytes per site per sweep over the measured copy bandwidth"},
+        "time_series": time_series,
         "update_plus_measurement": {"value": value_meas, "unit": UNIT, "steps": m_steps,
                                     "what": "sw_sweep(1) + sw_measure(energy, magnetisation, n_clusters) per step"},
+        "other_configs": other,
         "last_observables": obs,
         "label_equivalence_rounds_per_sweep": (stats["le_rounds_total"] / stats["sweeps"]) if args.label_equivalence else None,
         "paper_context": {"flips_per_ns_256xM2050_L65536": PAPER_FLIPS_PER_NS, "flips_per_ns_1xM2050_L4096": 0.232,
@@ -345,6 +473,36 @@ def run_gpu(args):
     if distributed:
         dist.destroy_process_group()
     return 0
+
+
+# ------------------------------------------------------------------------------------------------ control plane only (tests)
+
+def run_control_plane_only(args):
+    """Test hook (tests/test_bench_ranks.py): the rank plumbing of the N > 1 path on CPU -- gloo rendezvous, replica seeds,
+    sum of units over the max of times, ONE line from rank 0 -- with the GPU work replaced by fixed numbers.  It measures
+    nothing: `value` is null and the line says so."""
+    import torch.distributed as dist
+
+    from paper_1208_2080_b200 import replicas
+    rank, local_rank, world = rank_info()
+    if world > 1:
+        dist.init_process_group("gloo")
+    units, secs, rate = replicas.aggregate_throughput(1000.0 * args.steps, 1.0 + rank)
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "value": None, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                          "control_plane_only": True, "units_all_ranks": units, "max_seconds": secs,
+                          "replica_seeds": [replicas.replica_seed(1, r) for r in range(world)]}))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def spawn_ranks(args):
+    """`--gpus N` without a torchrun environment: start the N ranks ourselves, one per GPU, the way the driver would."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -359,16 +517,27 @@ def main():
                     help="SW_FLAG_LABEL_EQUIVALENCE: the paper's scan + analysis labeling (comparison variant, not the product path)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-baseline-L", type=int, default=4096)
-    ap.add_argument("--cpu-baseline-sweeps", type=int, default=4)
+    ap.add_argument("--no-other-configs", action="store_true")
+    ap.add_argument("--cpu-baseline-sweeps", type=int, default=20)
     ap.add_argument("--reference-L", type=int, default=2048)
+    ap.add_argument("--control-plane-only", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
+    if args.gpus < 1:
+        ap.error("--gpus must be >= 1")
     if args.impl == "reference":
         args.steps = 20 if args.steps is None else args.steps
         args.warmup = 5 if args.warmup is None else args.warmup
         return run_reference(args)
+    # N ranks: either torchrun started us (WORLD_SIZE must then agree with --gpus), or we start them ourselves
+    if "WORLD_SIZE" in os.environ:
+        if int(os.environ["WORLD_SIZE"]) != args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={os.environ['WORLD_SIZE']}: refusing to run a different number of ranks")
+    elif args.gpus > 1:
+        return spawn_ranks(args)
     args.steps = 40 if args.steps is None else args.steps
     args.warmup = 60 if args.warmup is None else args.warmup
+    if args.control_plane_only:
+        return run_control_plane_only(args)
     return run_gpu(args)
 
 

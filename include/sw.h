@@ -55,10 +55,22 @@ enum {
     SW_FLAG_FORCE_GENERIC = 1,  /* use the any-L reference kernels even where the tiled path applies     */
     SW_FLAG_LAZY_LABELS   = 2,  /* do not materialise canonical labels every sweep; flatten on demand
                                    (sw_get_labels / sw_measure of cluster sizes).  Same results.        */
-    SW_FLAG_LABEL_EQUIVALENCE = 4 /* comparison variant, any L: label step (2) with the "Label Equivalence" scheme
+    SW_FLAG_LABEL_EQUIVALENCE = 4,/* comparison variant, any L: label step (2) with the "Label Equivalence" scheme
                                    the paper uses (scanning + analysis kernels iterated until the
-                                   scanning changes nothing; the host reads a flag every round).  Same results,
-                                   much slower; sw_stats.le_rounds_* count the rounds (the paper: about 8.6).   */
+                                   scanning changes nothing; the host reads a flag every round, so in this mode
+                                   sw_sweep is SYNCHRONOUS).  Same results, much slower; sw_stats.le_rounds_*
+                                   count the rounds (the paper: about 8.6).                                     */
+    SW_FLAG_WS_CLUSTER_SIZES = 8, /* make the 4*L*L-byte scratch of sw_measure(largest_cluster) part of the
+                                   workspace (sw_workspace_bytes grows by it).  Without the flag the library
+                                   allocates that scratch itself, once, on the first call that needs it, and
+                                   keeps it until sw_destroy (sw_stats.device_bytes counts it).  Everything
+                                   else the library ever touches on the device lies inside the workspace.      */
+    SW_FLAG_PASS_COUNTERS = 16,   /* count the passes actually taken (sw_stats.merge_*, chase_*): instantiations of
+                                   the merge and flatten kernels with counters; off by default (a few per cent)  */
+    SW_FLAG_NO_CLUSTER_PATH = 32  /* lattices of at most 16 tiles (L <= 256, L % 64 == 0) run all the sweeps of a
+                                   call in ONE launch of a persistent kernel whose CTAs form one thread-block
+                                   cluster (sw_stats.path == 2); this flag keeps them on the three-kernels-per-
+                                   sweep path.  Same results.                                                   */
 };
 
 /* --- life cycle -------------------------------------------------------------------------------
@@ -71,7 +83,11 @@ int sw_create_ex(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed, 
 
 /* Device memory and stream lent by the caller (PyTorch in the Python binding).  `dev_ws` must be
  * a device pointer aligned to 256 bytes with at least sw_workspace_bytes(L, q, flags) bytes and
- * must outlive the context; `cuda_stream` is a cudaStream_t (NULL = the legacy default stream). */
+ * must outlive the context; `cuda_stream` is a cudaStream_t (NULL = the legacy default stream).
+ * The workspace holds everything: lattice arrays, the row ring of sw_sweep_measure, the staging
+ * buffer of sw_get_bonds (see SW_FLAG_WS_CLUSTER_SIZES for the one optional exception).
+ * Every call on a context runs on the device it was created on (the library switches to it and
+ * back), so contexts on several devices can be driven from one thread.                          */
 size_t sw_workspace_bytes(uint32_t L, uint32_t q, uint32_t flags);
 int sw_create_ws(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed, uint32_t flags,
                  void *dev_ws, size_t ws_bytes, void *cuda_stream);
@@ -107,6 +123,10 @@ int sw_measure(sw_ctx *ctx, uint64_t *energy_bonds, uint64_t *mag_counts,
  * (host uint64[n][3+q]) = energy_bonds, n_clusters, largest_cluster, mag_counts[0..q-1]
  * after sweep k.  Synchronises once at the end.                                                  */
 int sw_sweep_measure(sw_ctx *ctx, uint64_t n, uint64_t *out);
+/* The same with a choice of observables (BASELINE.json configs 3 and 4 want two of them each); columns that
+ * are not wanted are 0.  SW_OBS_LARGEST implies the cluster count.                                           */
+enum { SW_OBS_ENERGY = 1, SW_OBS_MAG = 2, SW_OBS_CLUSTERS = 4, SW_OBS_LARGEST = 8, SW_OBS_ALL = 15 };
+int sw_sweep_measure_ex(sw_ctx *ctx, uint64_t n, uint64_t *out, uint32_t what);
 
 /* --- read-back (all synchronise) ---------------------------------------------------------------*/
 int sw_get_spins(sw_ctx *ctx, uint8_t *dst /* host [L*L] */);
@@ -123,14 +143,27 @@ int sw_synchronize(sw_ctx *ctx);                   /* wait for the context strea
 
 /* --- introspection ------------------------------------------------------------------------------*/
 typedef struct sw_stats {
-    uint32_t path;              /* 0 = generic kernels, 1 = tiled path                              */
+    uint32_t path;              /* 0 = generic kernels, 1 = tiled path, 2 = tiled path as one persistent cluster kernel */
     uint32_t tile_w, tile_h;    /* tile shape of the tiled path                                     */
-    uint32_t kernels_per_sweep; /* kernel launches one sweep issues                                 */
+    uint32_t kernels_per_sweep; /* kernel launches one sweep issues (0 on path 2: one launch per call)    */
     uint64_t kernel_launches;   /* kernels launched by this context so far                          */
     uint64_t device_bytes;      /* device memory in use by this context                             */
     uint64_t sweeps;            /* sweeps issued so far                                             */
     uint64_t le_rounds_last;    /* SW_FLAG_LABEL_EQUIVALENCE: scanning + analysis rounds of the last sweep,   */
     uint64_t le_rounds_total;   /* ... and of all sweeps so far (the last round of a sweep changes nothing)   */
+    /* passes actually taken by the labeling (SW_FLAG_PASS_COUNTERS, tiled path; else 0), summed over all sweeps:
+     * the border merge (PAPER.md:66-68 one level down) is ONE pass whose cost is its find chains and lost races;
+     * the flatten ("tracks back the label variable until [it] remains unchanged") is one chase per
+     * tile-local root                                                                                          */
+    uint64_t merge_links;       /* border links united (after the duplicate filter)                          */
+    uint64_t merge_retries;     /* hooks that lost the race for a root and carried on                        */
+    uint64_t merge_hops;        /* parent loads of all finds of the merge                                    */
+    uint64_t chase_hops;        /* parent loads of all root chases of the flatten                            */
+    uint32_t max_merge_depth;   /* longest single find of the merge, in hops                                 */
+    uint32_t max_chase_depth;   /* longest single root chase of the flatten, in hops                         */
+    uint64_t bytes_moved;       /* algorithmic bytes of all sweeps so far: 14.5 B/site/sweep on the tiled path
+                                   (spins R+W 2, bond bits W+R 0.5, labels W, R, W 12),
+                                   10.5 with SW_FLAG_LAZY_LABELS; 0 on the generic path                       */
 } sw_stats;
 int sw_get_stats(sw_ctx *ctx, sw_stats *out);
 /* Time the kernels of the NEXT sweeps individually with CUDA events on the context stream:
@@ -139,6 +172,10 @@ int sw_get_stats(sw_ctx *ctx, sw_stats *out);
 #define SW_MAX_KERNEL_SLOTS 8
 int sw_profile_begin(sw_ctx *ctx);
 int sw_profile_end(sw_ctx *ctx, double ms_per_slot[SW_MAX_KERNEL_SLOTS], uint64_t launches_per_slot[SW_MAX_KERNEL_SLOTS]);
+/* Per-sweep device time of the region closed by the last sw_profile_end (first kernel's start to last kernel's
+ * end of each sweep, milliseconds): the time series SURVEY.md sec. 8(d) asks for.  *n = sweeps recorded; at most
+ * `cap` values are written.                                                                                      */
+int sw_profile_series(sw_ctx *ctx, double *ms_per_sweep, uint64_t cap, uint64_t *n);
 const char *sw_kernel_name(sw_ctx *ctx, int slot); /* NULL if the slot is unused                   */
 const char *sw_last_error(const sw_ctx *ctx);      /* text of the last failure on this context     */
 const char *sw_version(void);

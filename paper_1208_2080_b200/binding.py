@@ -15,6 +15,8 @@ import numpy as np
 OK, ERR_INVALID_ARG, ERR_OOM, ERR_CUDA, ERR_STATE = 0, 1, 2, 3, 4
 INIT_ORDERED, INIT_RANDOM = 0, 1
 FLAG_DEFAULT, FLAG_FORCE_GENERIC, FLAG_LAZY_LABELS, FLAG_LABEL_EQUIVALENCE = 0, 1, 2, 4
+FLAG_WS_CLUSTER_SIZES, FLAG_PASS_COUNTERS, FLAG_NO_CLUSTER_PATH = 8, 16, 32
+OBS_ENERGY, OBS_MAG, OBS_CLUSTERS, OBS_LARGEST, OBS_ALL = 1, 2, 4, 8, 15
 MAX_KERNEL_SLOTS = 8
 _STATUS = {1: "SW_ERR_INVALID_ARG", 2: "SW_ERR_OOM", 3: "SW_ERR_CUDA", 4: "SW_ERR_STATE"}
 
@@ -24,9 +26,9 @@ _lib = None
 # every symbol include/sw.h declares (tests check that the library exports them all)
 SYMBOLS = [
     "sw_create", "sw_create_ex", "sw_workspace_bytes", "sw_create_ws", "sw_destroy", "sw_init",
-    "sw_set_state", "sw_sweep", "sw_measure", "sw_sweep_measure", "sw_get_spins", "sw_get_labels",
+    "sw_set_state", "sw_sweep", "sw_measure", "sw_sweep_measure", "sw_sweep_measure_ex", "sw_get_spins", "sw_get_labels",
     "sw_get_bonds", "sw_get_rows", "sw_get_threshold", "sw_get_time", "sw_synchronize",
-    "sw_get_stats", "sw_profile_begin", "sw_profile_end", "sw_kernel_name", "sw_last_error",
+    "sw_get_stats", "sw_profile_begin", "sw_profile_end", "sw_profile_series", "sw_kernel_name", "sw_last_error",
     "sw_version",
 ]
 
@@ -41,7 +43,10 @@ class Stats(C.Structure):
     _fields_ = [("path", C.c_uint32), ("tile_w", C.c_uint32), ("tile_h", C.c_uint32),
                 ("kernels_per_sweep", C.c_uint32), ("kernel_launches", C.c_uint64),
                 ("device_bytes", C.c_uint64), ("sweeps", C.c_uint64),
-                ("le_rounds_last", C.c_uint64), ("le_rounds_total", C.c_uint64)]
+                ("le_rounds_last", C.c_uint64), ("le_rounds_total", C.c_uint64),
+                ("merge_links", C.c_uint64), ("merge_retries", C.c_uint64), ("merge_hops", C.c_uint64),
+                ("chase_hops", C.c_uint64), ("max_merge_depth", C.c_uint32), ("max_chase_depth", C.c_uint32),
+                ("bytes_moved", C.c_uint64)]
 
 
 def lib():
@@ -66,6 +71,7 @@ def lib():
     l.sw_sweep.argtypes = [vp, C.c_uint64]
     l.sw_measure.argtypes = [vp, u64p, u64p, u64p, u64p]
     l.sw_sweep_measure.argtypes = [vp, C.c_uint64, vp]
+    l.sw_sweep_measure_ex.argtypes = [vp, C.c_uint64, vp, C.c_uint32]
     l.sw_get_spins.argtypes = [vp, vp]
     l.sw_get_labels.argtypes = [vp, vp]
     l.sw_get_bonds.argtypes = [vp, vp]
@@ -76,6 +82,7 @@ def lib():
     l.sw_get_stats.argtypes = [vp, C.POINTER(Stats)]
     l.sw_profile_begin.argtypes = [vp]
     l.sw_profile_end.argtypes = [vp, C.POINTER(C.c_double), u64p]
+    l.sw_profile_series.argtypes = [vp, C.POINTER(C.c_double), C.c_uint64, u64p]
     l.sw_kernel_name.argtypes = [vp, C.c_int]; l.sw_kernel_name.restype = C.c_char_p
     l.sw_last_error.argtypes = [vp]; l.sw_last_error.restype = C.c_char_p
     l.sw_version.argtypes = []; l.sw_version.restype = C.c_char_p
@@ -165,9 +172,10 @@ class SwendsenWang:
         if largest: out["largest_cluster"] = int(big.value)
         return out
 
-    def sweep_measure(self, n):
+    def sweep_measure(self, n, what=OBS_ALL):
+        """n x (sweep, measure); columns: energy_bonds, n_clusters, largest_cluster, mag_counts[q]."""
         out = np.zeros((int(n), 3 + self.q), dtype=np.uint64)
-        self._chk(lib().sw_sweep_measure(self._h, int(n), out.ctypes.data), "sw_sweep_measure")
+        self._chk(lib().sw_sweep_measure_ex(self._h, int(n), out.ctypes.data, int(what)), "sw_sweep_measure")
         return out
 
     # -- read-back
@@ -212,7 +220,17 @@ class SwendsenWang:
     def stats(self):
         s = Stats()
         self._chk(lib().sw_get_stats(self._h, C.byref(s)), "sw_get_stats")
-        return {f: int(getattr(s, f)) for f, _ in Stats._fields_}
+        out = {f: int(getattr(s, f)) for f, _ in Stats._fields_}
+        out["path_name"] = {0: "generic", 1: "tiled", 2: "cluster (one persistent launch)"}.get(out["path"], "?")
+        return out
+
+    def profile_series(self):
+        """Per-sweep device milliseconds of the region closed by the last profile_end()."""
+        n = C.c_uint64()
+        self._chk(lib().sw_profile_series(self._h, None, 0, C.byref(n)), "sw_profile_series")
+        buf = (C.c_double * max(1, n.value))()
+        self._chk(lib().sw_profile_series(self._h, buf, n.value, C.byref(n)), "sw_profile_series")
+        return [float(buf[i]) for i in range(n.value)]
 
     def profile_begin(self):
         self._chk(lib().sw_profile_begin(self._h), "sw_profile_begin")
@@ -221,6 +239,7 @@ class SwendsenWang:
         ms = (C.c_double * MAX_KERNEL_SLOTS)()
         n = (C.c_uint64 * MAX_KERNEL_SLOTS)()
         self._chk(lib().sw_profile_end(self._h, ms, n), "sw_profile_end")
+        self.last_series = self.profile_series()
         out = {}
         for slot in range(MAX_KERNEL_SLOTS):
             name = lib().sw_kernel_name(self._h, slot)

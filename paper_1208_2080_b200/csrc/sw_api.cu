@@ -18,13 +18,14 @@
 #include "sw_observe.cuh"
 #include "sw_tiled.cuh"
 #include "sw_tile_blocks.cuh"
+#include "sw_cluster.cuh"
 
 namespace {
 
 using sw::Params;
 
 enum Slot { SLOT_TILE = 0, SLOT_MERGE = 1, SLOT_FLIP = 2, SLOT_G_BONDS = 3, SLOT_G_INIT = 4,
-            SLOT_G_UNION = 5, SLOT_G_FLATTEN = 6, SLOT_G_FLIP = 7 };
+            SLOT_G_UNION = 5, SLOT_G_FLATTEN = 6, SLOT_G_FLIP = 7 };   // the cluster path's one kernel is timed in SLOT_TILE
 const char *const kSlotNames[SW_MAX_KERNEL_SLOTS] = {
     "k_tile_blocks", "k_tile_merge", "k_tile_flip", "k_bonds_generic", "k_label_identity",
     "k_union_generic", "k_flatten_generic", "k_flip_generic"};
@@ -33,8 +34,12 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Plan {
-    size_t spins, bonds, labels, rootbits, border, edges, tile_clusters, draws, row, flag, total;   // byte offsets into the workspace
+    size_t spins, bonds, labels, rootbits, border, edges, tile_clusters, draws, row, flag, rows, stage, counters, sizes, total;   // byte offsets into the workspace
+    size_t rows_cap, stage_bytes;      // rows of the sw_sweep_measure ring; bytes of the sw_get_bonds staging buffer
 };
+
+constexpr uint32_t kAllFlags = SW_FLAG_FORCE_GENERIC | SW_FLAG_LAZY_LABELS | SW_FLAG_LABEL_EQUIVALENCE | SW_FLAG_WS_CLUSTER_SIZES |
+                               SW_FLAG_PASS_COUNTERS | SW_FLAG_NO_CLUSTER_PATH;
 
 bool tiled_ok(uint32_t L, uint32_t flags) { return (L % sw::kTile == 0) && !(flags & (SW_FLAG_FORCE_GENERIC | SW_FLAG_LABEL_EQUIVALENCE)); }
 
@@ -53,6 +58,16 @@ Plan make_plan(uint32_t L, uint32_t q, uint32_t flags)
     p.draws = off;  off = align_up(off + (tiled_ok(L, flags) ? (N / 32) * sizeof(uint2) : 0));   // one uint2 per 8 x 4 block
     p.row = off;    off = align_up(off + (3 + (size_t)q) * 8);
     p.flag = off;   off = align_up(off + 4);
+    // scratch the read-back / measurement calls need, owned by the context (no cudaMalloc behind the caller's back):
+    // a ring of observable rows for sw_sweep_measure, a staging buffer for sw_get_bonds, the pass counters of sw_get_stats
+    p.rows_cap = std::max<size_t>(16, std::min<size_t>(4096, (256u << 10) / ((3 + (size_t)q) * 8)));
+    p.rows = off;   off = align_up(off + p.rows_cap * (3 + (size_t)q) * 8);
+    p.stage_bytes = (size_t)std::min<uint64_t>(N, 32ull << 20);
+    p.stage = off;  off = align_up(off + p.stage_bytes);
+    p.counters = off; off = align_up(off + sizeof(sw::PassCounters));
+    // the 4N-byte cluster-size scratch of sw_measure(largest_cluster): part of the workspace only on request
+    // (SW_FLAG_WS_CLUSTER_SIZES); otherwise it is allocated once, on the first call that needs it
+    p.sizes = off;  off = align_up(off + ((flags & SW_FLAG_WS_CLUSTER_SIZES) ? N * 4 : 0));
     p.total = off;
     return p;
 }
@@ -64,6 +79,8 @@ struct sw_ctx {
     uint64_t N = 0, seed = 0, T = 0, t = 0;
     double K = 0;
     bool tiled = false, lazy = false, label_equiv = false;
+    bool cluster = false;                 // small lattice: all sweeps of a call in ONE launch of k_cluster_sweeps (sw_cluster.cuh)
+    uint32_t counts_per_tile = sw::kFlipThreads / 32;   // entries per tile the last flip left in d_tile_clusters
     uint64_t le_rounds_last = 0, le_rounds_total = 0;
     bool have_spins = false, have_labels = false, labels_flat = false;
     bool owns_ws = false, owns_stream = false;
@@ -79,14 +96,32 @@ struct sw_ctx {
     sw::TileBorder *d_border = nullptr;
     sw::TileEdges *d_edges = nullptr;
     unsigned long long *d_row = nullptr;
-    uint32_t *d_sizes = nullptr;          // lazily allocated 4N-byte scratch for cluster sizes
+    unsigned long long *d_rows = nullptr; // ring of observable rows for sw_sweep_measure (rows_cap rows)
+    size_t rows_cap = 0;
+    uint8_t *d_stage = nullptr;           // staging buffer of sw_get_bonds (stage_bytes)
+    size_t stage_bytes = 0;
+    sw::PassCounters *d_counters = nullptr;   // SW_FLAG_PASS_COUNTERS
+    bool count_passes = false;
+    uint32_t *d_sizes = nullptr;          // 4N-byte scratch for cluster sizes: in the workspace (SW_FLAG_WS_CLUSTER_SIZES) or
+    bool owns_sizes = false;              // allocated once by the first sw_measure(largest_cluster)
     uint64_t launches = 0, sweeps = 0;
     int num_sms = 148;
-    // profiling
+    // profiling: events are created once and reused (no cudaEventCreate inside a timed region after the first pass)
     bool profiling = false;
-    struct Ev { int slot; cudaEvent_t a, b; };
-    std::vector<Ev> events;
+    struct Ev { int slot; uint64_t sweep; cudaEvent_t a, b; };
+    std::vector<Ev> events;               // recorded since sw_profile_begin
+    std::vector<cudaEvent_t> event_pool;  // idle events
+    std::vector<double> series;           // per-sweep device time of the last profiled region (sw_profile_series)
     std::string err;
+};
+
+// every ABI call runs on the device the context was created on, whatever the caller's current device is
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(const sw_ctx *c) {
+        if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) cudaSetDevice(c->device); else prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
 namespace {
@@ -119,17 +154,6 @@ bool host_threshold(double K, uint64_t *T)
     return true;
 }
 
-// the per-sweep halves of Philox rounds 0 and 1 (philox_sweep in sw_common.cuh)
-void sweep_keys(const Params &P, uint32_t t, uint32_t k[3])
-{
-    const uint64_t m1t = 0xCD9E8D57ull * t;
-    const uint32_t a0 = (uint32_t)(m1t >> 32) ^ P.rk0[0], a1 = (uint32_t)m1t;
-    const uint64_t m0a = 0xD2511F53ull * a0;
-    k[0] = a1 ^ P.rk0[1];
-    k[1] = (uint32_t)(m0a >> 32) ^ P.rk1[1];
-    k[2] = (uint32_t)m0a;
-}
-
 Params make_params(const sw_ctx *c, uint64_t t)
 {
     Params P{};
@@ -144,8 +168,8 @@ Params make_params(const sw_ctx *c, uint64_t t)
     P.log2L = 0xFFFFFFFFu;
     for (uint32_t b = 0; b < 17; ++b) if ((1u << b) == c->L) P.log2L = b;
     P.divL_magic = ((1ull << 40) + c->L - 1) / c->L;
-    sweep_keys(P, P.t, P.pk_t);
-    sweep_keys(P, P.t + 1u, P.pk_n);
+    sw::sweep_keys(P, P.t, P.pk_t);
+    sw::sweep_keys(P, P.t + 1u, P.pk_n);
     return P;
 }
 
@@ -156,17 +180,80 @@ int grid_for(const sw_ctx *c, uint64_t items, int threads)
     return (int)(want < 1 ? 1 : (want > cap ? cap : want));
 }
 
+cudaEvent_t take_event(sw_ctx *c)
+{
+    cudaEvent_t e = nullptr;
+    if (!c->event_pool.empty()) { e = c->event_pool.back(); c->event_pool.pop_back(); return e; }
+    return cudaEventCreate(&e) == cudaSuccess ? e : nullptr;
+}
+
 struct Timed {
     sw_ctx *c; int slot; cudaEvent_t a = nullptr, b = nullptr;
     Timed(sw_ctx *c_, int slot_) : c(c_), slot(slot_) {
         c->launches += 1;
-        if (c->profiling && cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess)
-            cudaEventRecord(a, c->stream);
+        if (c->profiling && (a = take_event(c)) && (b = take_event(c))) cudaEventRecord(a, c->stream);
     }
     ~Timed() {
-        if (a && b) { cudaEventRecord(b, c->stream); c->events.push_back({slot, a, b}); }
+        if (a && b) { cudaEventRecord(b, c->stream); c->events.push_back({slot, c->sweeps, a, b}); }
     }
 };
+
+// Small lattices: n sweeps in one launch (sw_cluster.cuh).  what != 0: the observables of every sweep go to d_rows
+// (zeroed here), one row per sweep; the caller keeps n <= rows_cap then.
+int sweep_cluster(sw_ctx *c, uint64_t n, uint32_t what, unsigned long long *d_rows)
+{
+    const Params P = make_params(c, c->t);
+    const dim3 tgrid(c->L / sw::kTile, c->L / sw::kTile);
+    if (c->draws_t != c->t) {
+        c->launches += 1;
+        sw::k_draws<<<tgrid, 256, 0, c->stream>>>(c->d_draws, P);
+    }
+    if (what) SW_CUDA(c, cudaMemsetAsync(d_rows, 0, (size_t)n * (3 + (size_t)c->q) * 8, c->stream));
+    if ((what & SW_OBS_LARGEST) && !c->d_sizes) {
+        SW_CUDA(c, cudaMalloc(&c->d_sizes, c->N * 4));
+        c->owns_sizes = true;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = tgrid; cfg.blockDim = dim3(sw::kClusterThreads); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = tgrid.x; attr[0].val.clusterDim.y = tgrid.y; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    {
+        Timed tm(c, SLOT_TILE);
+        const uint32_t n32 = (uint32_t)n;
+        cudaError_t e = what ? cudaLaunchKernelEx(&cfg, sw::k_cluster_sweeps<true>, c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border,
+                                                  c->d_edges, c->d_draws, c->d_tile_clusters, P, n32, what, d_rows, c->d_sizes)
+                             : cudaLaunchKernelEx(&cfg, sw::k_cluster_sweeps<false>, c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border,
+                                                  c->d_edges, c->d_draws, c->d_tile_clusters, P, n32, 0u, (unsigned long long *)nullptr, (uint32_t *)nullptr);
+        if (e != cudaSuccess) return cuda_fail(c, e, "k_cluster_sweeps launch");
+    }
+    c->t += n; c->sweeps += n;
+    c->draws_t = c->t;
+    c->have_labels = true; c->labels_flat = true;
+    c->counts_per_tile = sw::kClusterThreads / 32;
+    return SW_OK;
+}
+
+// can a cluster of all the tiles be co-scheduled on this device?
+bool cluster_path_ok(sw_ctx *c)
+{
+    const unsigned tiles = (unsigned)(c->N / sw::kTileSites);
+    if (!c->tiled || tiles > sw::kClusterMaxTiles || c->lazy || c->count_passes) return false;
+    for (int m = 0; m < 2; ++m) {
+        const void *fn = m ? (const void *)sw::k_cluster_sweeps<true> : (const void *)sw::k_cluster_sweeps<false>;
+        if (tiles > 8 && cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) { cudaGetLastError(); return false; }
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(c->L / sw::kTile, c->L / sw::kTile); cfg.blockDim = dim3(sw::kClusterThreads);
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = cfg.gridDim.x; attr[0].val.clusterDim.y = cfg.gridDim.y; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        int n_clusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&n_clusters, fn, &cfg) != cudaSuccess || n_clusters < 1) { cudaGetLastError(); return false; }
+    }
+    return true;
+}
 
 // count_clusters: the flip kernel also counts the canonical roots (wanted for the last sweep before a measurement)
 int sweep_once(sw_ctx *c, bool count_clusters)
@@ -182,13 +269,16 @@ int sweep_once(sw_ctx *c, bool count_clusters)
         { Timed tm(c, SLOT_TILE);
           sw::k_tile_blocks<<<tgrid, sw::kBlkThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_edges, c->d_draws, P); }
         { Timed tm(c, SLOT_MERGE);
-          sw::k_tile_merge<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_edges, P, tiles); }
+          auto merge = c->count_passes ? sw::k_tile_merge<true> : sw::k_tile_merge<false>;
+          merge<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_edges, P, tiles, c->d_counters); }
         { Timed tm(c, SLOT_FLIP);
-          auto flip = c->lazy ? (count_clusters ? sw::k_tile_flip<false, true, true> : sw::k_tile_flip<false, true, false>)
+          auto flip = c->count_passes ? (c->lazy ? sw::k_tile_flip<false, true, true, true> : sw::k_tile_flip<true, true, true, true>)
+                    : c->lazy ? (count_clusters ? sw::k_tile_flip<false, true, true> : sw::k_tile_flip<false, true, false>)
                               : (count_clusters ? sw::k_tile_flip<true, true, true> : sw::k_tile_flip<true, true, false>);
-          flip<<<tgrid, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, c->d_draws); }
+          flip<<<tgrid, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, c->d_draws, c->d_counters); }
         c->draws_t = c->t + 1;           // the flip kernel made the draws of the next sweep on the side
         c->labels_flat = !c->lazy;
+        c->counts_per_tile = sw::kFlipThreads / 32;
     } else if (c->label_equiv) {
         // the loop of scanning and analysis kernels "is iterated up to the point when the information of
         // the labeling needs no more process of scanning function"; as in the paper the host looks at a flag every round
@@ -200,9 +290,10 @@ int sweep_once(sw_ctx *c, bool count_clusters)
         c->le_rounds_last = 0;
         for (uint32_t changed = 1; changed;) {
             SW_CUDA(c, cudaMemsetAsync(c->d_flag, 0, 4, c->stream));
-            c->launches += 2;
-            sw::k_le_scan<<<grid_for(c, c->N, th), th, 0, c->stream>>>(c->d_bonds, c->d_labels, P, c->d_flag);
-            sw::k_le_analysis<<<grid_for(c, c->N, th), th, 0, c->stream>>>(c->d_labels, P);
+            { Timed tm(c, SLOT_G_UNION);       // slot names in this mode: k_le_scan / k_le_analysis (sw_kernel_name)
+              sw::k_le_scan<<<grid_for(c, c->N, th), th, 0, c->stream>>>(c->d_bonds, c->d_labels, P, c->d_flag); }
+            { Timed tm(c, SLOT_G_FLATTEN);
+              sw::k_le_analysis<<<grid_for(c, c->N, th), th, 0, c->stream>>>(c->d_labels, P); }
             SW_CUDA(c, cudaMemcpyAsync(&changed, c->d_flag, 4, cudaMemcpyDeviceToHost, c->stream));
             SW_CUDA(c, cudaStreamSynchronize(c->stream));
             c->le_rounds_last += 1;
@@ -239,7 +330,7 @@ int ensure_flat(sw_ctx *c)
     const Params P = make_params(c, c->t);
     c->launches += 1;
     if (c->tiled)       // lazy mode: the forest of the last sweep is still in place (tile-local ids + root links)
-        sw::k_tile_flip<true, false, false><<<dim3(c->L / sw::kTile, c->L / sw::kTile), sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, nullptr);
+        sw::k_tile_flip<true, false, false><<<dim3(c->L / sw::kTile, c->L / sw::kTile), sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, nullptr, nullptr);
     else
         sw::k_flatten_generic<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_labels, P);
     SW_CUDA(c, cudaGetLastError());
@@ -257,7 +348,7 @@ int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m
     if ((want & 4u) && c->tiled) {      // the flip kernel of the last sweep left one count per tile: no pass over labels[]
         want &= ~4u;
         c->launches += 1;
-        const unsigned tiles = (unsigned)(c->N / sw::kTileSites) * (sw::kFlipThreads / 32);   // one count per warp of the flip kernel
+        const unsigned tiles = (unsigned)(c->N / sw::kTileSites) * c->counts_per_tile;   // one count per warp of the last flip
         sw::k_sum_tile_clusters<<<grid_for(c, tiles, sw::kObsThreads), sw::kObsThreads, 0, c->stream>>>(c->d_tile_clusters, tiles, row);
     }
     if (want) {
@@ -272,7 +363,10 @@ int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m
             const int rc = ensure_flat(c);
             if (rc != SW_OK) return rc;
         }
-        if (!c->d_sizes) SW_CUDA(c, cudaMalloc(&c->d_sizes, c->N * 4));
+        if (!c->d_sizes) {               // not part of the workspace (no SW_FLAG_WS_CLUSTER_SIZES): allocated once, kept until sw_destroy
+            SW_CUDA(c, cudaMalloc(&c->d_sizes, c->N * 4));
+            c->owns_sizes = true;
+        }
         SW_CUDA(c, cudaMemsetAsync(c->d_sizes, 0, c->N * 4, c->stream));
         c->launches += 2;
         sw::k_cluster_sizes<<<grid_for(c, (c->N + 15) / 16, 256), 256, 0, c->stream>>>(c->d_labels, c->d_sizes, P);
@@ -295,7 +389,7 @@ int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed,
     *out = nullptr;
     uint64_t T = 0;
     if (L < 2 || L > 65536 || q < 2 || q > 255 || !host_threshold(K, &T)) return SW_ERR_INVALID_ARG;
-    if (flags & ~(uint32_t)(SW_FLAG_FORCE_GENERIC | SW_FLAG_LAZY_LABELS | SW_FLAG_LABEL_EQUIVALENCE)) return SW_ERR_INVALID_ARG;
+    if (flags & ~kAllFlags) return SW_ERR_INVALID_ARG;
     sw_ctx *c = new (std::nothrow) sw_ctx();
     if (!c) return SW_ERR_OOM;
     c->L = L; c->q = q; c->K = K; c->seed = seed; c->T = T; c->flags = flags;
@@ -327,6 +421,19 @@ int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed,
     c->d_draws = (uint2 *)(c->ws + plan.draws);
     c->d_row = (unsigned long long *)(c->ws + plan.row);
     c->d_flag = (uint32_t *)(c->ws + plan.flag);
+    c->d_rows = (unsigned long long *)(c->ws + plan.rows); c->rows_cap = plan.rows_cap;
+    c->d_stage = c->ws + plan.stage; c->stage_bytes = plan.stage_bytes;
+    c->d_counters = (sw::PassCounters *)(c->ws + plan.counters);
+    c->count_passes = (flags & SW_FLAG_PASS_COUNTERS) != 0 && c->tiled;
+    c->cluster = !(flags & SW_FLAG_NO_CLUSTER_PATH) && cluster_path_ok(c);
+    if (flags & SW_FLAG_WS_CLUSTER_SIZES) c->d_sizes = (uint32_t *)(c->ws + plan.sizes);
+    if (cudaMemsetAsync(c->d_counters, 0, sizeof(sw::PassCounters), c->stream) != cudaSuccess) {
+        cudaGetLastError();
+        if (c->owns_stream) cudaStreamDestroy(c->stream);
+        if (c->owns_ws) cudaFree(c->ws);
+        delete c;
+        return SW_ERR_CUDA;
+    }
     *out = c;
     return SW_OK;
 }
@@ -362,9 +469,11 @@ int sw_create_ws(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed, 
 void sw_destroy(sw_ctx *c)
 {
     if (!c) return;
+    DeviceGuard dg(c);
     cudaStreamSynchronize(c->stream);
     for (auto &ev : c->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
-    if (c->d_sizes) cudaFree(c->d_sizes);
+    for (auto &ev : c->event_pool) cudaEventDestroy(ev);
+    if (c->d_sizes && c->owns_sizes) cudaFree(c->d_sizes);
     if (c->owns_ws) cudaFree(c->ws);
     if (c->owns_stream) cudaStreamDestroy(c->stream);
     delete c;
@@ -373,6 +482,7 @@ void sw_destroy(sw_ctx *c)
 int sw_init(sw_ctx *c, int mode)
 {
     if (!c) return SW_ERR_INVALID_ARG;
+    DeviceGuard dg(c);
     if (mode == SW_INIT_ORDERED) {
         SW_CUDA(c, cudaMemsetAsync(c->d_spins, 0, c->N, c->stream));
     } else if (mode == SW_INIT_RANDOM) {
@@ -388,6 +498,7 @@ int sw_init(sw_ctx *c, int mode)
 int sw_set_state(sw_ctx *c, const uint8_t *src, uint64_t t)
 {
     if (!c || !src || t > 0xFFFFFFFFull) return fail(c, SW_ERR_INVALID_ARG, "sw_set_state: bad argument");
+    DeviceGuard dg(c);
     SW_CUDA(c, cudaMemcpyAsync(c->d_spins, src, c->N, cudaMemcpyHostToDevice, c->stream));
     SW_CUDA(c, cudaMemsetAsync(c->d_flag, 0, 4, c->stream));
     const Params P = make_params(c, 0);
@@ -407,6 +518,17 @@ int sw_sweep(sw_ctx *c, uint64_t n)
     if (!c) return SW_ERR_INVALID_ARG;
     if (!c->have_spins) return fail(c, SW_ERR_STATE, "sw_sweep: no spins (call sw_init or sw_set_state)");
     if (c->t + n > 0x100000000ull) return fail(c, SW_ERR_STATE, "sw_sweep: sweep counter would pass 2^32");
+    DeviceGuard dg(c);
+    if (c->cluster) {                    // small lattice: all the sweeps in one launch (chunks keep the 32-bit loop counter safe)
+        for (uint64_t done = 0; done < n;) {
+            const uint64_t m = std::min<uint64_t>(n - done, 1u << 20);
+            const int rc = sweep_cluster(c, m, 0, nullptr);
+            if (rc != SW_OK) return rc;
+            done += m;
+        }
+        SW_CUDA(c, cudaGetLastError());
+        return SW_OK;
+    }
     for (uint64_t k = 0; k < n; ++k) {
         const int rc = sweep_once(c, k + 1 == n);
         if (rc != SW_OK) return rc;
@@ -419,6 +541,7 @@ int sw_measure(sw_ctx *c, uint64_t *energy_bonds, uint64_t *mag_counts, uint64_t
 {
     if (!c) return SW_ERR_INVALID_ARG;
     if (!c->have_spins) return fail(c, SW_ERR_STATE, "sw_measure: no spins");
+    DeviceGuard dg(c);
     const int rc = enqueue_observe(c, c->d_row, energy_bonds != nullptr, mag_counts != nullptr,
                                    n_clusters != nullptr || largest_cluster != nullptr, largest_cluster != nullptr);
     if (rc != SW_OK) return rc;
@@ -433,22 +556,26 @@ int sw_measure(sw_ctx *c, uint64_t *energy_bonds, uint64_t *mag_counts, uint64_t
     return SW_OK;
 }
 
-int sw_sweep_measure(sw_ctx *c, uint64_t n, uint64_t *out)
+int sw_sweep_measure(sw_ctx *c, uint64_t n, uint64_t *out) { return sw_sweep_measure_ex(c, n, out, SW_OBS_ALL); }
+
+int sw_sweep_measure_ex(sw_ctx *c, uint64_t n, uint64_t *out, uint32_t what)
 {
-    if (!c || (!out && n)) return SW_ERR_INVALID_ARG;
+    if (!c || (!out && n) || (what & ~(uint32_t)SW_OBS_ALL)) return SW_ERR_INVALID_ARG;
     if (!c->have_spins) return fail(c, SW_ERR_STATE, "sw_sweep_measure: no spins");
     if (c->t + n > 0x100000000ull) return fail(c, SW_ERR_STATE, "sw_sweep_measure: sweep counter would pass 2^32");
     if (n == 0) return SW_OK;
+    DeviceGuard dg(c);
     const size_t stride = 3 + (size_t)c->q;
-    const uint64_t chunk_max = 4096;
-    unsigned long long *d_rows = nullptr;
-    SW_CUDA(c, cudaMalloc(&d_rows, (size_t)(n < chunk_max ? n : chunk_max) * stride * 8));
+    const uint64_t chunk_max = c->rows_cap;              // the ring of rows is part of the context's workspace
+    unsigned long long *d_rows = c->d_rows;
     int rc = SW_OK;
     for (uint64_t done = 0; done < n && rc == SW_OK;) {
         const uint64_t m = (n - done < chunk_max) ? n - done : chunk_max;
-        for (uint64_t k = 0; k < m && rc == SW_OK; ++k) {
-            rc = sweep_once(c, true);
-            if (rc == SW_OK) rc = enqueue_observe(c, d_rows + k * stride, true, true, true, true);
+        if (c->cluster) rc = sweep_cluster(c, m, what, d_rows);
+        else for (uint64_t k = 0; k < m && rc == SW_OK; ++k) {
+            rc = sweep_once(c, (what & (SW_OBS_CLUSTERS | SW_OBS_LARGEST)) != 0);
+            if (rc == SW_OK) rc = enqueue_observe(c, d_rows + k * stride, (what & SW_OBS_ENERGY) != 0, (what & SW_OBS_MAG) != 0,
+                                                  (what & (SW_OBS_CLUSTERS | SW_OBS_LARGEST)) != 0, (what & SW_OBS_LARGEST) != 0);
         }
         if (rc == SW_OK) {
             cudaError_t e = cudaMemcpyAsync(out + done * stride, d_rows, (size_t)m * stride * 8, cudaMemcpyDeviceToHost, c->stream);
@@ -458,7 +585,6 @@ int sw_sweep_measure(sw_ctx *c, uint64_t n, uint64_t *out)
         if (rc == SW_OK) for (uint64_t k = 0; k < m; ++k) fix_row(c, out + (done + k) * stride);
         done += m;
     }
-    cudaFree(d_rows);
     return rc;
 }
 
@@ -466,6 +592,7 @@ int sw_get_rows(sw_ctx *c, int what, uint32_t y0, uint32_t nrows, void *dst)
 {
     if (!c || !dst || (uint64_t)y0 + nrows > c->L) return fail(c, SW_ERR_INVALID_ARG, "sw_get_rows: bad argument");
     if (nrows == 0) return SW_OK;
+    DeviceGuard dg(c);
     const uint64_t first = (uint64_t)y0 * c->L, count = (uint64_t)nrows * c->L;
     if (what == 0) {
         if (!c->have_spins) return fail(c, SW_ERR_STATE, "no spins");
@@ -477,19 +604,17 @@ int sw_get_rows(sw_ctx *c, int what, uint32_t y0, uint32_t nrows, void *dst)
         SW_CUDA(c, cudaMemcpyAsync(dst, c->d_labels + first, count * 4, cudaMemcpyDeviceToHost, c->stream));
     } else if (what == 2) {
         if (!c->have_labels) return fail(c, SW_ERR_STATE, "no bonds: no sweep since sw_init");
-        const uint64_t chunk = 64ull << 20;
-        uint8_t *tmp = nullptr;
-        SW_CUDA(c, cudaMalloc(&tmp, (size_t)(count < chunk ? count : chunk)));
+        const uint64_t chunk = c->stage_bytes;           // staging buffer owned by the context
+        uint8_t *tmp = c->d_stage;
         for (uint64_t done = 0; done < count;) {
             const uint64_t m = (count - done < chunk) ? count - done : chunk;
             c->launches += 1;
             sw::k_expand_bonds<<<grid_for(c, m, 256), 256, 0, c->stream>>>(c->d_bonds, tmp, first + done, m);
             cudaError_t e = cudaMemcpyAsync((uint8_t *)dst + done, tmp, m, cudaMemcpyDeviceToHost, c->stream);
             if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-            if (e != cudaSuccess) { cudaFree(tmp); return cuda_fail(c, e, "sw_get_bonds copy"); }
+            if (e != cudaSuccess) return cuda_fail(c, e, "sw_get_bonds copy");
             done += m;
         }
-        cudaFree(tmp);
     } else return fail(c, SW_ERR_INVALID_ARG, "sw_get_rows: unknown array");
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
     return SW_OK;
@@ -516,6 +641,7 @@ int sw_get_time(sw_ctx *c, uint64_t *t)
 int sw_synchronize(sw_ctx *c)
 {
     if (!c) return SW_ERR_INVALID_ARG;
+    DeviceGuard dg(c);
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
     SW_CUDA(c, cudaGetLastError());
     return SW_OK;
@@ -524,21 +650,33 @@ int sw_synchronize(sw_ctx *c)
 int sw_get_stats(sw_ctx *c, sw_stats *out)
 {
     if (!c || !out) return SW_ERR_INVALID_ARG;
-    out->path = c->tiled ? 1u : 0u;
+    out->path = c->cluster ? 2u : c->tiled ? 1u : 0u;
     out->tile_w = out->tile_h = c->tiled ? sw::kTile : 0u;
-    out->kernels_per_sweep = c->tiled ? 3u : c->label_equiv ? (uint32_t)(3u + 2u * c->le_rounds_last) : (c->lazy ? 4u : 5u);
+    out->kernels_per_sweep = c->cluster ? 0u : c->tiled ? 3u : c->label_equiv ? (uint32_t)(3u + 2u * c->le_rounds_last) : (c->lazy ? 4u : 5u);
     out->kernel_launches = c->launches;
-    out->device_bytes = c->ws_bytes + (c->d_sizes ? c->N * 4 : 0);
+    out->device_bytes = c->ws_bytes + (c->owns_sizes ? c->N * 4 : 0);
     out->sweeps = c->sweeps;
     out->le_rounds_last = c->le_rounds_last;
     out->le_rounds_total = c->le_rounds_total;
+    out->merge_links = out->merge_retries = out->merge_hops = out->chase_hops = 0;
+    out->max_merge_depth = out->max_chase_depth = 0;
+    if (c->count_passes) {
+        DeviceGuard dg(c);
+        sw::PassCounters pc;
+        SW_CUDA(c, cudaMemcpyAsync(&pc, c->d_counters, sizeof(pc), cudaMemcpyDeviceToHost, c->stream));
+        SW_CUDA(c, cudaStreamSynchronize(c->stream));
+        out->merge_links = pc.merge_links; out->merge_retries = pc.merge_retries; out->merge_hops = pc.merge_hops;
+        out->chase_hops = pc.chase_hops; out->max_merge_depth = pc.max_merge_depth; out->max_chase_depth = pc.max_chase_depth;
+    }
+    // algorithmic bytes the sweeps so far had to move (spins R + W, bond bits W, label passes)
+    out->bytes_moved = (uint64_t)((double)c->sweeps * (double)c->N * (c->tiled ? (c->lazy ? 10.5 : 14.5) : 0.0));
     return SW_OK;
 }
 
 int sw_profile_begin(sw_ctx *c)
 {
     if (!c) return SW_ERR_INVALID_ARG;
-    for (auto &ev : c->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+    for (auto &ev : c->events) { c->event_pool.push_back(ev.a); c->event_pool.push_back(ev.b); }
     c->events.clear();
     c->profiling = true;
     return SW_OK;
@@ -548,24 +686,43 @@ int sw_profile_end(sw_ctx *c, double ms_per_slot[SW_MAX_KERNEL_SLOTS], uint64_t 
 {
     if (!c || !ms_per_slot || !launches_per_slot) return SW_ERR_INVALID_ARG;
     c->profiling = false;
+    DeviceGuard dg(c);
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
     for (int s = 0; s < SW_MAX_KERNEL_SLOTS; ++s) { ms_per_slot[s] = 0.0; launches_per_slot[s] = 0; }
+    c->series.clear();
+    for (size_t i = 0; i < c->events.size();) {          // per sweep: first kernel's start to last kernel's end
+        size_t j = i;
+        while (j + 1 < c->events.size() && c->events[j + 1].sweep == c->events[i].sweep) ++j;
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, c->events[i].a, c->events[j].b) == cudaSuccess) c->series.push_back(ms);
+        i = j + 1;
+    }
     for (auto &ev : c->events) {
         float ms = 0.f;
         if (cudaEventElapsedTime(&ms, ev.a, ev.b) == cudaSuccess) { ms_per_slot[ev.slot] += ms; launches_per_slot[ev.slot] += 1; }
-        cudaEventDestroy(ev.a); cudaEventDestroy(ev.b);
+        c->event_pool.push_back(ev.a); c->event_pool.push_back(ev.b);
     }
     c->events.clear();
+    return SW_OK;
+}
+
+int sw_profile_series(sw_ctx *c, double *ms_per_sweep, uint64_t cap, uint64_t *n)
+{
+    if (!c || !n || (!ms_per_sweep && cap)) return SW_ERR_INVALID_ARG;
+    *n = c->series.size();
+    for (uint64_t i = 0; i < cap && i < c->series.size(); ++i) ms_per_sweep[i] = c->series[i];
     return SW_OK;
 }
 
 const char *sw_kernel_name(sw_ctx *c, int slot)
 {
     if (!c || slot < 0 || slot >= SW_MAX_KERNEL_SLOTS) return nullptr;
+    if (c->cluster) return slot == SLOT_TILE ? "k_cluster_sweeps" : nullptr;
     const bool tiled_slot = slot <= SLOT_FLIP;
     if (tiled_slot != c->tiled) return nullptr;
     if (slot == SLOT_G_FLATTEN && c->lazy) return nullptr;
-    if (c->label_equiv && (slot == SLOT_G_UNION || slot == SLOT_G_FLATTEN)) return nullptr;   // scan / analysis rounds are not timed per slot
+    if (c->label_equiv && slot == SLOT_G_UNION) return "k_le_scan";         // all rounds of a sweep accumulate in these two slots
+    if (c->label_equiv && slot == SLOT_G_FLATTEN) return "k_le_analysis";
     return kSlotNames[slot];
 }
 

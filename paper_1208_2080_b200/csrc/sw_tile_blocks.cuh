@@ -119,22 +119,29 @@ __device__ __forceinline__ uint32_t slot_of4(uint32_t W, uint32_t c)
     return (((W >> c) & 0x01010101u) * kDecodeMul) >> 24;
 }
 
-__global__ void __launch_bounds__(kBlkThreads, 9)
-k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
-              uint32_t *__restrict__ labels, uint16_t *__restrict__ rootbits,
-              TileBorder *__restrict__ border, TileEdges *__restrict__ edges, const uint2 *__restrict__ draws, Params P)
+// The body of the tile kernel for tile (tx, ty) of a piece of the lattice, run by kBlkThreads threads.
+//   kSuper     the piece is a sub-lattice of the super-lattice (label values global, addresses local: `dom`);
+//              false: the whole lattice, dom is not looked at
+//   kCoherent  see ld_in
+//   Bar        the CTA-wide barrier of those kBlkThreads threads
+template <bool kSuper, bool kCoherent, class Bar>
+__device__ __forceinline__ void
+tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8_t *spins, uint32_t *bonds,
+                 uint32_t *labels, uint16_t *rootbits, TileBorder *border, TileEdges *edges, const uint2 *draws,
+                 const Params &P, const Dom &dom)
 {
-    __shared__ BlkShared S;
-
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t bx = tid & 7u, by = tid >> 3;
-    const uint32_t L = P.L, tiles_x = L >> 6;
-    const uint32_t ty = blockIdx.y, tx = blockIdx.x, tile = ty * tiles_x + tx;   // grid = (tiles_x, tiles_x): no division
+    const uint32_t L = kSuper ? dom.Lg : P.L;                  // row stride of label values (global site indices)
+    const uint32_t W = kSuper ? dom.W : P.L;                   // row stride of the arrays
+    const uint32_t tiles_x = W >> 6;
+    const uint32_t tile = ty * tiles_x + tx;
     const uint32_t X0 = tx << 6, Y0 = ty << 6;
     const uint32_t x0 = X0 + (bx << 3), y0 = Y0 + (by << 2);
-    const uint32_t origin = Y0 * L + X0;                       // global index of the tile's first site
+    const uint32_t origin = kSuper ? (dom.oy + Y0) * L + dom.ox + X0 : Y0 * L + X0;   // global index of the tile's first site
     const uint32_t idbase = (by << 8) + (bx << 3);             // tile-local id of my first site
     const uint32_t i0 = origin + idbase / 64u * L + (bx << 3); // global index of my first site (mod 2^32 exact: N <= 2^32)
+    const uint32_t a0 = kSuper ? y0 * W + x0 : i0;             // its array offset
 
     // -- union-find array: identity
     {
@@ -151,20 +158,29 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
     uint2 s[5];
 #pragma unroll
     for (int r = 0; r < 4; ++r)
-        s[r] = *reinterpret_cast<const uint2 *>(spins + (uint64_t)(y0 + r) * L + x0);
+        s[r] = ld_in<kCoherent>(reinterpret_cast<const uint2 *>(spins + (uint64_t)(y0 + r) * W + x0));
     s[4].x = __shfl_down_sync(0xFFFFFFFFu, s[0].x, 8);
     s[4].y = __shfl_down_sync(0xFFFFFFFFu, s[0].y, 8);
     if ((lane >> 3) == 3u) {
-        const uint32_t yd = (y0 + 4u == L) ? 0u : y0 + 4u;
-        s[4] = *reinterpret_cast<const uint2 *>(spins + (uint64_t)yd * L + x0);
+        if (kSuper && y0 + 4u == dom.H) {                      // row 0 of the piece below
+            s[4] = ld_in<true>(reinterpret_cast<const uint2 *>(dom.down + x0));
+        } else {
+            const uint32_t yd = (!kSuper && y0 + 4u == L) ? 0u : y0 + 4u;
+            s[4] = ld_in<kCoherent>(reinterpret_cast<const uint2 *>(spins + (uint64_t)yd * W + x0));
+        }
     }
     uint32_t nx = __byte_perm(__byte_perm(s[0].x, s[1].x, 0x0040), __byte_perm(s[2].x, s[3].x, 0x0040), 0x5410);
     nx = __shfl_down_sync(0xFFFFFFFFu, nx, 1);                // column 0 of the block on my right, one byte per row
     if (bx == 7u) {
-        const uint32_t xr = (X0 + kTile == L) ? 0u : X0 + kTile;
         nx = 0;
+        if (kSuper && X0 + kTile == W) {                       // column 0 of the piece on the right
 #pragma unroll
-        for (int r = 0; r < 4; ++r) nx |= (uint32_t)spins[(uint64_t)(y0 + r) * L + xr] << (8 * r);
+            for (int r = 0; r < 4; ++r) nx |= (uint32_t)ld_in<true>(dom.right + (uint64_t)(y0 + r) * dom.right_W) << (8 * r);
+        } else {
+            const uint32_t xr = (!kSuper && X0 + kTile == L) ? 0u : X0 + kTile;
+#pragma unroll
+            for (int r = 0; r < 4; ++r) nx |= (uint32_t)ld_in<kCoherent>(spins + (uint64_t)(y0 + r) * W + xr) << (8 * r);
+        }
     }
 
     // -- step (1): a bond is active iff the spins are equal and its draw is below the threshold
@@ -173,7 +189,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
         // The threshold tests of this sweep's draws were made ahead of time (tile_draw_masks in sw_tiled.cuh: by the flip
         // kernel of the previous sweep while it waited for its loads, or by k_draws): bit 8r + c of dm.x / dm.y says
         // whether the right / down draw of my site (r, c) is below the threshold.
-        const uint2 dm = draws[tile * kBlkThreads + tid];
+        const uint2 dm = ld_in<kCoherent>(draws + tile * kBlkThreads + tid);
         if (P.q == 2u) {                                       // spins are 0 / 1: "equal" is bit 0 of the XNOR (pack4 looks at bit 0 only)
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
@@ -209,10 +225,10 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
         for (int h = 0; h < 2; ++h) {
             const uint32_t r = 2u * odd + h, sel = r | ((4u + r) << 4);
             const uint32_t word = __byte_perm(__byte_perm(Re, Ro, sel), __byte_perm(De, Do, sel), 0x5410);
-            bonds[(i0 + r * L) >> 4] = word;
+            bonds[(a0 + r * W) >> 4] = word;
         }
     }
-    __syncthreads();                                           // B1: parent[], edge[] visible
+    Bar::sync();                                               // B1: parent[], edge[] visible
 
     // -- the bonds that leave the tile (warp 0): right bonds of block column 7, down bonds of block row 15
     if (warp == 0) {
@@ -330,7 +346,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
             }
         }
     };
-    const bool crowded = __syncthreads_or(n > (uint32_t)kBlkBufSlot);   // B2: seeds of all blocks visible
+    const bool crowded = Bar::sync_or(n > (uint32_t)kBlkBufSlot);   // B2: seeds of all blocks visible
     uint32_t *const buf = &S.list[kBlkBufSlot][0] + warp * kBlkExtraCap;
     if (!crowded) {
         walk_links([&](uint32_t a, uint32_t b) { S.parent[a] = (uint16_t)b; },
@@ -338,7 +354,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
     } else {
         walk_links([&](uint32_t a, uint32_t b) { S.parent[a] = (uint16_t)b; }, [](uint32_t, uint32_t) {});
     }
-    __syncthreads();                                           // B3: the plain-store forest is complete
+    Bar::sync();                                               // B3: the plain-store forest is complete
     if (!crowded) {
         const uint32_t n_warp = S.n_extra[warp];
         for (uint32_t k = lane; k < n_warp; k += 32) {
@@ -348,7 +364,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
     } else {
         walk_links([](uint32_t, uint32_t) {}, [&](uint32_t a, uint32_t b) { unite_s16(S.parent, a, b); });
     }
-    __syncthreads();                                           // B4: no hooks happen any more
+    Bar::sync();                                               // B4: no hooks happen any more
 
     // -- every component: its root (chase; compress my own entry only) and root flag
     uint32_t rootm = ~todo;                                    // a site without any bond is its own cluster
@@ -389,7 +405,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
                 lab[c] = ((rootm >> (8 * r + c)) & 1u) ? self + c : v;
             }
         }
-        uint4 *lp = reinterpret_cast<uint4 *>(labels + (uint64_t)(y0 + r) * L + x0);
+        uint4 *lp = reinterpret_cast<uint4 *>(labels + (uint64_t)(y0 + r) * W + x0);
         lp[0] = make_uint4(lab[0], lab[1], lab[2], lab[3]);
         lp[1] = make_uint4(lab[4], lab[5], lab[6], lab[7]);
         col_l[r] = lab[0];
@@ -409,7 +425,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             const uint32_t r = 2u * odd + h;
-            rootbits[(i0 + r * L) >> 4] = (uint16_t)(((me >> (8 * r)) & 0xFFu) | (((mo >> (8 * r)) & 0xFFu) << 8));
+            rootbits[(a0 + r * W) >> 4] = (uint16_t)(((me >> (8 * r)) & 0xFFu) | (((mo >> (8 * r)) & 0xFFu) << 8));
         }
     }
     if (bx == 0u || bx == 7u) {                               // left / right column of the tile
@@ -422,6 +438,30 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
         }
         *reinterpret_cast<uint4 *>((bx == 0u ? edges[tile].left : edges[tile].right) + 4u * by) = make_uint4(g[0], g[1], g[2], g[3]);
     }
+}
+
+struct CtaBar {
+    static __device__ __forceinline__ void sync() { __syncthreads(); }
+    static __device__ __forceinline__ bool sync_or(bool p) { return __syncthreads_or(p) != 0; }
+};
+
+__global__ void __launch_bounds__(kBlkThreads, 9)
+k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
+              uint32_t *__restrict__ labels, uint16_t *__restrict__ rootbits,
+              TileBorder *__restrict__ border, TileEdges *__restrict__ edges, const uint2 *__restrict__ draws, Params P)
+{
+    __shared__ BlkShared S;
+    tile_blocks_body<false, false, CtaBar>(S, blockIdx.x, blockIdx.y, spins, bonds, labels, rootbits, border, edges, draws, P, Dom{});   // grid = (tiles_x, tiles_x): no division
+}
+
+// the same for one sub-lattice of the super-lattice (sw_super.cu); grid = (W / 64, H / 64)
+__global__ void __launch_bounds__(kBlkThreads, 9)
+k_tile_blocks_super(const uint8_t *spins, uint32_t *__restrict__ bonds,
+                    uint32_t *__restrict__ labels, uint16_t *__restrict__ rootbits,
+                    TileBorder *__restrict__ border, TileEdges *__restrict__ edges, const uint2 *__restrict__ draws, Params P, Dom dom)
+{
+    __shared__ BlkShared S;
+    tile_blocks_body<true, false, CtaBar>(S, blockIdx.x, blockIdx.y, spins, bonds, labels, rootbits, border, edges, draws, P, dom);
 }
 
 }  // namespace sw

@@ -58,15 +58,16 @@ __device__ __forceinline__ uint32_t shift_in_not_below(uint32_t mask, uint32_t d
 
 // 256 threads per tile: thread u makes the draws of rows 2h, 2h + 1 (h = u % 2) of block u / 2: one Philox call per
 // site pair (words: right, down, right, down), last pair first so that the bits are shifted in in order.
-__device__ __forceinline__ void tile_draw_masks(uint2 *__restrict__ draws, uint32_t tile, uint32_t origin, uint32_t u,
-                                                const uint32_t (&pk)[3], const Params &P)
+// `origin` = global index of the tile's first site, `Lg` = global row stride (the draws are keyed by the global site)
+__device__ __forceinline__ void tile_draw_masks(uint2 *draws, uint32_t tile, uint32_t origin, uint32_t u,
+                                                const uint32_t (&pk)[3], const Params &P, const uint32_t Lg)
 {
     const uint32_t b = u >> 1, h = u & 1u, bx = b & 7u, by = b >> 3;
     const uint32_t above = ~P.thr_m1;                          // 2^32 - T (T >= 1; T = 0 is masked by thr_any)
     uint32_t off_r = 0, off_d = 0;                             // the draws that are NOT below the threshold
 #pragma unroll
     for (int rr = 1; rr >= 0; --rr) {
-        const uint32_t pair0 = (origin + ((by << 2) + 2u * h + rr) * P.L + (bx << 3)) >> 1;
+        const uint32_t pair0 = (origin + ((by << 2) + 2u * h + rr) * Lg + (bx << 3)) >> 1;
 #pragma unroll
         for (int p = 3; p >= 0; --p) {
             const uint4 d = philox_sweep(pair0 + p, kPurposeBond, pk, P);
@@ -87,7 +88,14 @@ k_draws(uint2 *__restrict__ draws, Params P)
 {
     const uint32_t tiles_x = P.L >> 6;
     const uint32_t ty = blockIdx.y, tx = blockIdx.x, tile = ty * tiles_x + tx;   // grid = (tiles_x, tiles_x): no division
-    tile_draw_masks(draws, tile, (ty << 6) * P.L + (tx << 6), threadIdx.x, P.pk_t, P);
+    tile_draw_masks(draws, tile, (ty << 6) * P.L + (tx << 6), threadIdx.x, P.pk_t, P, P.L);
+}
+
+__global__ void __launch_bounds__(256)
+k_draws_super(uint2 *__restrict__ draws, Params P, Dom dom)
+{
+    const uint32_t tile = blockIdx.y * (dom.W >> 6) + blockIdx.x;
+    tile_draw_masks(draws, tile, (dom.oy + (blockIdx.y << 6)) * dom.Lg + dom.ox + (blockIdx.x << 6), threadIdx.x, P.pk_t, P, dom.Lg);
 }
 
 // ---- kernel 2: merge across tile borders -------------------------------------------------------
@@ -99,41 +107,54 @@ k_draws(uint2 *__restrict__ draws, Params P)
 
 constexpr int kMergeTiles = 4;
 
-__global__ void __launch_bounds__(kMergeThreads)
-k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, const TileEdges *__restrict__ edges,
-             Params P, uint32_t n_tiles)
-{
-    __shared__ uint2 s_link[kMergeTiles * kMergeThreads];
-    __shared__ uint32_t s_n;
+struct MergeShared {
+    uint2 link[kMergeTiles * kMergeThreads];
+    uint32_t n;
+};
 
+// The links of tiles [tile_begin, tile_end) (at most kMergeTiles of them), by kMergeThreads threads.
+//   kSuper: borders that leave the piece are NOT united here (the inter-domain merge of sw_super.cu does that,
+//   PAPER.md:66-68); label values are global, addresses local (DomAddr).
+template <bool kStats, bool kSuper, bool kCoherent, class Bar>
+__device__ __forceinline__ void
+tile_merge_body(MergeShared &S, uint32_t *labels, const TileBorder *border, const TileEdges *edges, const Params &P, const Dom &dom,
+                const uint32_t tile_begin, const uint32_t tile_end, PassCounters *counters)
+{
     const uint32_t b = threadIdx.x, lane = b & 31u;
-    const uint32_t tiles_x = P.L >> 6;
-    if (b == 0) s_n = 0;
-    __syncthreads();
+    const uint32_t tiles_x = (kSuper ? dom.W : P.L) >> 6, tiles_y = (kSuper ? dom.H : P.L) >> 6;
+    if (b == 0) S.n = 0;
+    Bar::sync();
 
     uint32_t lu[kMergeTiles], lv[kMergeTiles];
     bool on[kMergeTiles];
 #pragma unroll
     for (int i = 0; i < kMergeTiles; ++i) {
-        const uint32_t tile = blockIdx.x * kMergeTiles + i;
+        const uint32_t tile = tile_begin + i;
         on[i] = false; lu[i] = 0; lv[i] = 0;
-        if (tile < n_tiles) {
+        if (tile < tile_end) {
             const uint32_t ty = tile / tiles_x, tx = tile - ty * tiles_x;
-            const TileBorder rec = border[tile];
+            TileBorder rec;
+            if (kCoherent) {
+                const ulonglong2 v = __ldcg(reinterpret_cast<const ulonglong2 *>(border + tile));
+                rec.right_col = v.x; rec.bottom_row = v.y;
+            } else rec = border[tile];
             const uint32_t *pu, *pv;
             unsigned long long mask;
             uint32_t k;
+            bool inside = true;
             if (b < kTile) {                                 // right column -- left column of the tile on the right
                 k = b; mask = rec.right_col;
                 pu = edges[tile].right + k;
                 pv = edges[(tx + 1 == tiles_x) ? tile - tx : tile + 1].left + k;
+                if (kSuper) inside = tx + 1 != tiles_x;
             } else {                                         // bottom row -- top row of the tile below
                 k = b - kTile; mask = rec.bottom_row;
                 pu = edges[tile].bottom + k;
-                pv = edges[(ty + 1 == tiles_x) ? tx : tile + tiles_x].top + k;
+                pv = edges[(ty + 1 == tiles_y) ? tx : tile + tiles_x].top + k;
+                if (kSuper) inside = ty + 1 != tiles_y;
             }
-            on[i] = (mask >> k) & 1ull;
-            if (on[i]) { lu[i] = *pu; lv[i] = *pv; }
+            on[i] = inside && ((mask >> k) & 1ull);
+            if (on[i]) { lu[i] = ld_in<kCoherent>(pu); lv[i] = ld_in<kCoherent>(pv); }
         }
     }
 #pragma unroll
@@ -145,16 +166,49 @@ k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, const Tile
         const bool keep = on[i] && !dup;
         const uint32_t m = __ballot_sync(0xFFFFFFFFu, keep);
         uint32_t base = 0;
-        if (lane == 0 && m) base = atomicAdd(&s_n, (uint32_t)__popc(m));
+        if (lane == 0 && m) base = atomicAdd(&S.n, (uint32_t)__popc(m));
         base = __shfl_sync(0xFFFFFFFFu, base, 0);
-        if (keep) s_link[base + __popc(m & ((1u << lane) - 1u))] = make_uint2(lu[i], lv[i]);
+        if (keep) S.link[base + __popc(m & ((1u << lane) - 1u))] = make_uint2(lu[i], lv[i]);
     }
-    __syncthreads();
-    const uint32_t n = s_n;
+    Bar::sync();
+    const uint32_t n = S.n;
+    uint32_t st[3] = {0, 0, 0};                              // kStats: hops, longest find, lost races
     for (uint32_t k = b; k < n; k += kMergeThreads) {
-        const uint2 e = s_link[k];
-        unite(labels, e.x, e.y);
+        const uint2 e = S.link[k];
+        if (kSuper) unite<kStats, DomAddr>(labels, e.x, e.y, st, DomAddr(dom));
+        else unite<kStats>(labels, e.x, e.y, st);
     }
+    if (kStats) {
+        const uint32_t hops = __reduce_add_sync(0xFFFFFFFFu, st[0]), deep = __reduce_max_sync(0xFFFFFFFFu, st[1]);
+        const uint32_t lost = __reduce_add_sync(0xFFFFFFFFu, st[2]);
+        if (lane == 0) {
+            atomicAdd(&counters->merge_hops, (unsigned long long)hops);
+            atomicAdd(&counters->merge_retries, (unsigned long long)lost);
+            atomicMax(&counters->max_merge_depth, deep);
+        }
+        if (b == 0) atomicAdd(&counters->merge_links, (unsigned long long)n);
+    }
+}
+
+struct MergeBar {
+    static __device__ __forceinline__ void sync() { __syncthreads(); }
+};
+
+template <bool kStats>
+__global__ void __launch_bounds__(kMergeThreads)
+k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, const TileEdges *__restrict__ edges,
+             Params P, uint32_t n_tiles, PassCounters *__restrict__ counters)
+{
+    __shared__ MergeShared S;
+    tile_merge_body<kStats, false, false, MergeBar>(S, labels, border, edges, P, Dom{}, blockIdx.x * kMergeTiles, n_tiles, counters);
+}
+
+__global__ void __launch_bounds__(kMergeThreads)
+k_tile_merge_super(uint32_t *labels, const TileBorder *__restrict__ border, const TileEdges *__restrict__ edges,
+                   Params P, Dom dom, uint32_t n_tiles)
+{
+    __shared__ MergeShared S;
+    tile_merge_body<false, true, false, MergeBar>(S, labels, border, edges, P, dom, blockIdx.x * kMergeTiles, n_tiles, nullptr);
 }
 
 // ---- kernel 3: flatten to the canonical root + flip --------------------------------------------
@@ -170,56 +224,71 @@ k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, const Tile
 // x = 4 (l % 16) .. + 3 of row kFlipRows w + 2k + l / 16.
 
 constexpr int kFlipThreads = 256;                                // (tile_draw_masks is written for 256 threads per tile)
-constexpr int kFlipAcc = (int)kTileSites / (4 * kFlipThreads);   // 16-byte accesses per thread
-constexpr int kFlipRows = 2 * kFlipAcc;                          // tile rows per warp
 
+template <int NT>
+struct FlipShared {
+    static constexpr int kAcc = (int)kTileSites / (4 * NT);       // 16-byte accesses per thread
+    static constexpr int kRows = 2 * kAcc;                       // tile rows per warp
+    uint32_t root[kTileSites];                                   // per tile-local root: its canonical root
+    uint8_t state[kTileSites];                                   // per tile-local root: the new state
+    uint16_t list[NT / 32][kRows * kTile];                       // per warp: the tile-local roots of its rows
+};
+
+// The body of the flip kernel for tile (tx, ty), run by NT threads.
 // kLabels: write the canonical labels back (eager mode, or the on-demand flatten of lazy mode);
 // kSpins: draw and write the new spins; kCount: leave the number of canonical roots per warp in tile_clusters[]
 // (n_clusters of sw_measure without a pass over labels[]; costs 3 % of the kernel, so only the last sweep of a call does it).
-template <bool kLabels, bool kSpins, bool kCount>
-__global__ void __launch_bounds__(kFlipThreads, 6)
-k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__restrict__ spins, Params P,
-            uint32_t *__restrict__ tile_clusters, uint2 *__restrict__ next_draws)
+// kSuper: one sub-lattice of the super-lattice: label values global, addresses local; a chase ends at a root OR at the
+// first link that leaves the piece (after the resolve pass of sw_super.cu such a link points at the canonical root).
+// pk_t / pk_n: philox_sweep constants of this sweep and the next (Params::pk_t / pk_n, or made on the device).
+template <bool kLabels, bool kSpins, bool kCount, bool kStats, bool kSuper, int NT, class Bar>
+__device__ __forceinline__ void
+tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t *labels, const uint16_t *rootbits, uint8_t *spins,
+               const Params &P, const uint32_t (&pk_t)[3], const uint32_t (&pk_n)[3], const Dom &dom,
+               uint32_t *tile_clusters, uint2 *next_draws, PassCounters *counters)
 {
-    __shared__ uint32_t s_root[kTileSites];                   // per tile-local root: its canonical root
-    __shared__ uint8_t s_state[kTileSites];                   // per tile-local root: the new state
-    __shared__ uint16_t s_list[kFlipThreads / 32][kFlipRows * kTile];   // per warp: the tile-local roots of its rows
-
+    constexpr int kAcc = FlipShared<NT>::kAcc, kRows = FlipShared<NT>::kRows;
     const uint32_t tid = threadIdx.x;
     const uint32_t lane = tid & 31u, warp = tid >> 5;
-    const uint32_t L = P.L, tiles_x = L >> 6;
-    const uint32_t ty = blockIdx.y, tx = blockIdx.x, tile = ty * tiles_x + tx;   // grid = (tiles_x, tiles_x): no division
-    const uint32_t origin = (ty << 6) * L + (tx << 6);
+    const uint32_t L = kSuper ? dom.Lg : P.L;                  // row stride of label values (global site indices)
+    const uint32_t W = kSuper ? dom.W : P.L;                   // row stride of the arrays
+    const uint32_t tiles_x = W >> 6;
+    const uint32_t tile = ty * tiles_x + tx;
+    const uint32_t origin = kSuper ? (dom.oy + (ty << 6)) * L + dom.ox + (tx << 6) : (ty << 6) * L + (tx << 6);
     const uint32_t x4 = (lane & 15u) << 2;                     // my first column inside the tile
-    const uint32_t yk0 = warp * kFlipRows + (lane >> 4);       // my tile row for k = 0 (k-th: + 2k)
+    const uint32_t yk0 = warp * kRows + (lane >> 4);           // my tile row for k = 0 (k-th: + 2k)
     const uint32_t i00 = origin + yk0 * L + x4;                // global index of my first site for k = 0
+    const uint32_t a00 = kSuper ? ((ty << 6) + yk0) * W + (tx << 6) + x4 : i00;   // its array offset
 
     // -- phase A: everything this tile needs from HBM is requested at once: my labels and root flags.
     //    A tile-local root's own entry is its link into the global forest (itself if the merge never hooked
     //    it), so the first step of every chase comes out of this coalesced load instead of a scattered one.
     //    What a site needs afterwards is the tile-local id of its root (12 bits; its own id if it is a root): two per
     //    register, so the 16 sites of a thread cost 8 registers across the chases instead of 16.
-    uint32_t ids[2 * kFlipAcc];
+    uint32_t ids[2 * kAcc];
     uint32_t work = 0;                                         // bit 4k + j: my site j of access k is a tile-local root
-    uint4 lq[kFlipAcc];
-    uint32_t rq[kFlipAcc];
+    uint4 lq[kAcc];
+    uint32_t rq[kAcc];
 #pragma unroll
-    for (int k = 0; k < kFlipAcc; ++k) {
-        const uint32_t i0 = i00 + 2 * k * L;
-        lq[k] = __ldcg(reinterpret_cast<const uint4 *>(labels + i0));
-        rq[k] = rootbits[i0 >> 4];
+    for (int k = 0; k < kAcc; ++k) {
+        const uint32_t o = a00 + 2 * k * W;
+        lq[k] = __ldcg(reinterpret_cast<const uint4 *>(labels + o));
+        rq[k] = rootbits[o >> 4];
     }
     // while those loads are on their way: the bond draws of the NEXT sweep for this tile (pure arithmetic, see above)
-    if (kSpins && next_draws) tile_draw_masks(next_draws, tile, origin, tid, P.pk_n, P);
+    if (kSpins && next_draws) {
 #pragma unroll
-    for (int k = 0; k < kFlipAcc; ++k) {
+        for (int u = 0; u < 256; u += NT) tile_draw_masks(next_draws, tile, origin, tid + u, pk_n, P, L);
+    }
+#pragma unroll
+    for (int k = 0; k < kAcc; ++k) {
         const uint4 l = lq[k];
         const uint32_t lab[4] = {l.x, l.y, l.z, l.w};
         const uint32_t rb = (rq[k] >> (x4 & 12u)) & 15u;
         const uint32_t id0 = ((yk0 + 2 * k) << 6) + x4;
         // where the chase of a root starts: its own entry.  All four entries are stored with one 16-byte store; the
         // entries of sites that are not roots are never read (every lookup goes to a root's id).
-        *reinterpret_cast<uint4 *>(&s_root[id0]) = l;
+        *reinterpret_cast<uint4 *>(&S.root[id0]) = l;
         uint32_t id[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) id[j] = ((rb >> j) & 1u) ? id0 + j : lab[j];
@@ -243,41 +312,79 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
         while (w) {
             const uint32_t j = __ffs(w) - 1u;
             w &= w - 1u;
-            s_list[warp][pos++] = (uint16_t)(idb + ((j >> 2) << 7) + (j & 3u));
+            S.list[warp][pos++] = (uint16_t)(idb + ((j >> 2) << 7) + (j & 3u));
         }
         __syncwarp();
         // ... and gives each ONE chase and ONE new state (step (3)), 32 roots at a time
+        uint32_t hops_all = 0, hops_max = 0;                   // kStats
         for (uint32_t k = lane; k < n_warp; k += 32) {
-            const uint32_t id = s_list[warp][k];
+            const uint32_t id = S.list[warp][k];
             const uint32_t self = origin + (id >> 6) * L + (id & 63u);
-            const uint32_t g = find_root_halving_from(labels, self, s_root[id]);
-            s_root[id] = g;
-            if (kSpins) s_state[id] = (uint8_t)flip_state(g, P);
+            uint32_t hops = 1;                                 // the first hop came with the coalesced load of phase A
+            uint32_t g;
+            if (kSuper) {
+                const DomAddr addr(dom);
+                uint32_t a = self;
+                g = S.root[id];
+                while (g != a && addr.mine(g)) { a = g; g = ld_label(labels, a, addr); }
+            } else {
+                g = find_root_halving_from<kStats>(labels, self, S.root[id], &hops);
+            }
+            if (kStats) { hops_all += hops; hops_max = max(hops_max, hops); }
+            S.root[id] = g;
+            if (kSpins) S.state[id] = (uint8_t)flip_state(g, pk_t, P);
+        }
+        if (kStats) {
+            hops_all = __reduce_add_sync(0xFFFFFFFFu, hops_all);
+            hops_max = __reduce_max_sync(0xFFFFFFFFu, hops_max);
+            if (lane == 0) { atomicAdd(&counters->chase_hops, (unsigned long long)hops_all); atomicMax(&counters->max_chase_depth, hops_max); }
         }
     }
-    __syncthreads();
+    Bar::sync();
 
     // -- phase C: every site looks up (canonical root, new state) of its tile-local root
     uint32_t canon = 0;                                        // clusters whose smallest site is one of mine (for sw_measure)
 #pragma unroll
-    for (int k = 0; k < kFlipAcc; ++k) {
-        const uint32_t i0 = i00 + 2 * k * L;
+    for (int k = 0; k < kAcc; ++k) {
+        const uint32_t i0 = i00 + 2 * k * L, o = a00 + 2 * k * W;
         uint32_t st = 0, lab[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const uint32_t id = (j & 1) ? ids[2 * k + (j >> 1)] >> 16 : ids[2 * k + (j >> 1)] & 0xFFFFu;
-            lab[j] = s_root[id];
+            lab[j] = S.root[id];
             if (kCount) canon += (lab[j] == i0 + j);           // a canonical root is its own label
-            if (kSpins) st |= (uint32_t)s_state[id] << (8 * j);
+            if (kSpins) st |= (uint32_t)S.state[id] << (8 * j);
         }
-        if (kSpins) *reinterpret_cast<uint32_t *>(spins + i0) = st;
+        if (kSpins) *reinterpret_cast<uint32_t *>(spins + o) = st;
         if (kLabels)
-            *reinterpret_cast<uint4 *>(labels + i0) = make_uint4(lab[0], lab[1], lab[2], lab[3]);
+            *reinterpret_cast<uint4 *>(labels + o) = make_uint4(lab[0], lab[1], lab[2], lab[3]);
     }
     if (kCount) {
         canon = __reduce_add_sync(0xFFFFFFFFu, canon);
-        if (lane == 0) tile_clusters[tile * (kFlipThreads / 32) + warp] = canon;
+        if (lane == 0) tile_clusters[tile * (NT / 32) + warp] = canon;
     }
+}
+
+template <bool kLabels, bool kSpins, bool kCount, bool kStats = false>
+__global__ void __launch_bounds__(kFlipThreads, 6)
+k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__restrict__ spins, Params P,
+            uint32_t *__restrict__ tile_clusters, uint2 *__restrict__ next_draws, PassCounters *__restrict__ counters = nullptr)
+{
+    __shared__ FlipShared<kFlipThreads> S;
+    tile_flip_body<kLabels, kSpins, kCount, kStats, false, kFlipThreads, MergeBar>(
+        S, blockIdx.x, blockIdx.y, labels, rootbits, spins, P, P.pk_t, P.pk_n, Dom{}, tile_clusters, next_draws, counters);   // grid = (tiles_x, tiles_x): no division
+}
+
+// one sub-lattice of the super-lattice; grid = (W / 64, H / 64).  `spins` is read by the neighbours' tile kernels of the
+// next sweep (their halo), never by this kernel.
+template <bool kLabels, bool kSpins, bool kCount>
+__global__ void __launch_bounds__(kFlipThreads, 6)
+k_tile_flip_super(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *spins, Params P, Dom dom,
+                  uint32_t *__restrict__ tile_clusters, uint2 *__restrict__ next_draws)
+{
+    __shared__ FlipShared<kFlipThreads> S;
+    tile_flip_body<kLabels, kSpins, kCount, false, true, kFlipThreads, MergeBar>(
+        S, blockIdx.x, blockIdx.y, labels, rootbits, spins, P, P.pk_t, P.pk_n, dom, tile_clusters, next_draws, nullptr);
 }
 
 }  // namespace sw

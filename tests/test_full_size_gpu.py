@@ -7,8 +7,9 @@ checks (a) sampled outputs the oracle computes one by one -- bond draws, new sta
 and (b) properties that hold at any size and pin the rest: every label is a fixed-point root <= the site,
 an active bond joins equal labels, no bond joins different spins, all members of a label carry the
 root's state, and the observables equal a plain numpy count over the whole lattice.  The complete
-single-step comparison with the oracle at L = 65536 is `test_L65536_full_transition_vs_oracle`
-(opt-in: SW_RUN_HUGE=1; its last recorded run is in DESIGN.md).
+single-step comparison with the oracle at L = 65536 is `test_L65536_one_late_transition_vs_oracle` (default-on, one
+late t, about 6 minutes) and `test_L65536_full_transition_vs_oracle` (opt-in: SW_RUN_HUGE=1, t = 1 and a second late t;
+its last recorded run is under profiles/).
 """
 import os
 
@@ -122,18 +123,30 @@ def test_full_size_properties_and_sampled_outputs(name):
     assert 1 <= m["largest_cluster"] <= N
 
 
-@pytest.mark.huge
-@pytest.mark.skipif(os.environ.get("SW_RUN_HUGE") != "1", reason="~15 min of host CPU and ~35 GiB of host RAM; set SW_RUN_HUGE=1")
-def test_L65536_full_transition_vs_oracle():
+def _transition_L65536(ts):
     """Single-step transition check: GPU spins after sweep t-1 are handed to the oracle,
-    one oracle sweep, everything compared with the GPU's sweep t.  t = 1 and a late t."""
+    one oracle sweep (about 5 minutes and 35 GiB of host RAM at 2^32 sites), everything compared with the GPU's sweep t."""
     c = wl.CONFIGS["c5_L65536_q2"]
     gpu = SwendsenWang(c["L"], c["q"], c["K"], c["seed"])
     cpu = Oracle(c["L"], c["q"], c["K"], c["seed"])
     gpu.init(c["start"])
-    for warm in (1, int(os.environ.get("SW_HUGE_LATE_T", "40"))):
+    for warm in ts:
         gpu.sweep(warm - gpu.get_time())
         t = gpu.get_time()
         cpu.set_state(gpu.get_spins(), t)
         gpu.sweep(1); cpu.sweep(1)
         full_compare(gpu, cpu, f"L=65536 sweep {t}")
+
+
+def test_L65536_one_late_transition_vs_oracle():
+    """Default-on: the headline lattice (2^32 sites) in the launch configuration bench.py times, one complete sweep at a
+    late t (t = 30: giant cluster present, long hooked chains) compared bit for bit with the oracle -- every bond,
+    canonical label, spin and observable.  Catches 32-bit index arithmetic that only wraps at N = 2^32."""
+    _transition_L65536([30])
+
+
+@pytest.mark.huge
+@pytest.mark.skipif(os.environ.get("SW_RUN_HUGE") != "1", reason="~15 min of host CPU and ~35 GiB of host RAM; set SW_RUN_HUGE=1")
+def test_L65536_full_transition_vs_oracle():
+    """Opt-in: two more transitions (t = 1 and a second late t)."""
+    _transition_L65536([1, int(os.environ.get("SW_HUGE_LATE_T", "40"))])

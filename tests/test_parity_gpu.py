@@ -75,7 +75,8 @@ def test_tiled_path_other_temperatures_from_an_ordered_start(L, K):
     run_pair(L, 2, K, seed=3, start="ordered", sweeps=3)
 
 
-@pytest.mark.parametrize("flags", [sw.FLAG_LAZY_LABELS, sw.FLAG_FORCE_GENERIC, sw.FLAG_FORCE_GENERIC | sw.FLAG_LAZY_LABELS])
+@pytest.mark.parametrize("flags", [sw.FLAG_LAZY_LABELS, sw.FLAG_FORCE_GENERIC, sw.FLAG_FORCE_GENERIC | sw.FLAG_LAZY_LABELS,
+                                   sw.FLAG_NO_CLUSTER_PATH])
 def test_flag_variants_give_identical_results(flags):
     run_pair(128, 3, wl.k_critical(3), seed=5, start="random", sweeps=3, flags=flags)
     run_pair(192, 2, wl.k_critical(2), seed=5, start="ordered", sweeps=3, flags=flags)
@@ -180,8 +181,50 @@ def test_randomised_configurations():
         gpu.close(); cpu.close()
 
 
+def test_cluster_path_is_selected_for_small_lattices():
+    # L <= 256: all the sweeps of a call in ONE launch of the persistent cluster kernel (path 2)
+    for L in (64, 128, 192, 256):
+        g = SwendsenWang(L, 2, 0.5, 1)
+        g.init("ordered")
+        g.sweep(5)
+        g.sweep(2)
+        g.synchronize()
+        st = g.stats()
+        assert st["path"] == 2 and st["path_name"].startswith("cluster") and st["sweeps"] == 7
+        assert st["kernel_launches"] == 3                     # k_draws once + one launch per sw_sweep call
+    g = SwendsenWang(320, 2, 0.5, 1)                           # 25 tiles: more than one cluster holds
+    assert g.stats()["path"] == 1
+
+
+@pytest.mark.parametrize("L", [64, 128, 192, 256])
+@pytest.mark.parametrize("q", [2, 3, 10])
+def test_three_kernel_path_at_small_sizes(L, q):
+    # the same sizes on the three-kernels-per-sweep path the big lattices use
+    run_pair(L, q, wl.k_critical(q), seed=2, start="random", sweeps=3, flags=sw.FLAG_NO_CLUSTER_PATH)
+
+
+def test_cluster_path_many_sweeps_in_one_launch_and_series():
+    # 200 sweeps in one launch == 200 oracle sweeps; the series call == the oracle's series, for every choice of observables
+    c = wl.CONFIGS["c1_L256_q2"]
+    gpu, cpu = SwendsenWang(c["L"], c["q"], c["K"], c["seed"]), Oracle(c["L"], c["q"], c["K"], c["seed"])
+    gpu.init(c["start"]); cpu.init(c["start"])
+    gpu.sweep(200); cpu.sweep(200)
+    compare_after_sweep(gpu, cpu, "(200 sweeps in one launch)")
+    want = cpu.sweep_measure(30)
+    got = np.concatenate([gpu.sweep_measure(10), gpu.sweep_measure(10, sw.OBS_ENERGY | sw.OBS_MAG), gpu.sweep_measure(10, sw.OBS_CLUSTERS)])
+    assert np.array_equal(got[:10], want[:10])
+    assert np.array_equal(got[10:20, 0], want[10:20, 0]) and np.array_equal(got[10:20, 3:], want[10:20, 3:]) and not got[10:20, 1:3].any()
+    assert np.array_equal(got[20:, 1], want[20:, 1]) and not got[20:, 0].any() and not got[20:, 2:].any()
+    compare_after_sweep(gpu, cpu, "(after the series calls)")
+    for q, K in ((3, wl.k_critical(3)), (37, 2.5)):
+        gpu, cpu = SwendsenWang(192, q, K, 6), Oracle(192, q, K, 6)
+        gpu.init("random"); cpu.init("random")
+        assert np.array_equal(gpu.sweep_measure(12), cpu.sweep_measure(12)), q
+        compare_after_sweep(gpu, cpu, f"(series, q={q})")
+
+
 def test_tiled_path_is_selected_and_counts_kernels():
-    g = SwendsenWang(128, 2, 0.5, 1)
+    g = SwendsenWang(128, 2, 0.5, 1, flags=sw.FLAG_NO_CLUSTER_PATH)
     g.init("ordered")
     g.sweep(3)
     g.synchronize()
@@ -331,9 +374,58 @@ def test_state_machine_and_errors():
 def test_profile_slots():
     g = SwendsenWang(256, 2, wl.k_critical(2), 1)
     g.init("random")
+    g.profile_begin(); g.sweep(5); prof = g.profile_end()
+    assert set(prof) == {"k_cluster_sweeps"} and prof["k_cluster_sweeps"]["launches"] == 1
+    g = SwendsenWang(256, 2, wl.k_critical(2), 1, flags=sw.FLAG_NO_CLUSTER_PATH)
+    g.init("random")
     g.sweep(2)
     g.profile_begin()
     g.sweep(5)
     prof = g.profile_end()
     assert set(prof) == {"k_tile_blocks", "k_tile_merge", "k_tile_flip"}
     assert all(v["launches"] == 5 and v["ms"] > 0 for v in prof.values())
+
+
+def test_pass_counters_and_workspace_scratch_flags():
+    # SW_FLAG_PASS_COUNTERS: counting instantiations of the merge / flatten kernels -- same results, counters filled;
+    # SW_FLAG_WS_CLUSTER_SIZES: the cluster-size scratch is part of the workspace (no allocation by the library)
+    L, q, K = 256, 2, wl.k_critical(2)
+    flags = sw.FLAG_PASS_COUNTERS | sw.FLAG_WS_CLUSTER_SIZES
+    gpu, cpu = SwendsenWang(L, q, K, 8, flags=flags), Oracle(L, q, K, 8)
+    gpu.init("ordered"); cpu.init("ordered")
+    for k in range(4):
+        gpu.sweep(1); cpu.sweep(1)
+        compare_after_sweep(gpu, cpu, f"(pass counters, sweep {k})")
+    st = gpu.stats()
+    assert st["merge_links"] > 0 and st["merge_hops"] >= 2 * st["merge_links"] and st["chase_hops"] > 0
+    assert 1 <= st["max_merge_depth"] < 64 and 1 <= st["max_chase_depth"] < 64
+    assert st["bytes_moved"] == int(4 * L * L * 14.5)
+    assert st["device_bytes"] == sw.workspace_bytes(L, q, flags)          # largest_cluster was measured: nothing allocated on the side
+    plain = SwendsenWang(L, q, K, 8)
+    plain.init("ordered"); plain.sweep(2)
+    s0 = plain.stats()
+    assert s0["merge_links"] == 0 and s0["chase_hops"] == 0 and s0["device_bytes"] == sw.workspace_bytes(L, q)
+    plain.measure()
+    assert plain.stats()["device_bytes"] == sw.workspace_bytes(L, q) + 4 * L * L   # documented lazy scratch
+
+
+def test_sweep_measure_mask_and_series():
+    L, q, K = 192, 3, wl.k_critical(3)
+    gpu, cpu = SwendsenWang(L, q, K, 4), Oracle(L, q, K, 4)
+    gpu.init("random"); cpu.init("random")
+    want = cpu.sweep_measure(6)
+    got = gpu.sweep_measure(3, sw.OBS_ENERGY | sw.OBS_MAG)
+    assert np.array_equal(got[:, 0], want[:3, 0]) and np.array_equal(got[:, 3:], want[:3, 3:]) and not got[:, 1:3].any()
+    got = gpu.sweep_measure(3, sw.OBS_CLUSTERS | sw.OBS_LARGEST)
+    assert np.array_equal(got[:, 1:3], want[3:, 1:3]) and not got[:, 0].any() and not got[:, 3:].any()
+    assert np.array_equal(gpu.get_spins(), cpu.get_spins())
+    big = SwendsenWang(320, q, K, 4)                            # three kernels per sweep: one series entry per sweep
+    big.init("random")
+    big.profile_begin(); big.sweep(5); big.profile_end()
+    assert len(big.last_series) == 5 and all(v > 0 for v in big.last_series)
+    gpu.profile_begin(); gpu.sweep(5); gpu.profile_end()      # cluster path: the 5 sweeps are one launch
+    assert len(gpu.last_series) == 1 and gpu.last_series[0] > 0
+    many = SwendsenWang(64, 2, 0.5, 1)                          # more rows than the context's ring holds: chunked
+    ref = Oracle(64, 2, 0.5, 1)
+    many.init("random"); ref.init("random")
+    assert np.array_equal(many.sweep_measure(5000)[::97], ref.sweep_measure(5000)[::97])
