@@ -180,6 +180,44 @@ const char *sw_kernel_name(sw_ctx *ctx, int slot); /* NULL if the slot is unused
 const char *sw_last_error(const sw_ctx *ctx);      /* text of the last failure on this context     */
 const char *sw_version(void);
 
+/* --- the super-lattice decomposition ---------------------------------------------------------
+ * The L x L lattice cut into gx x gy equal sub-lattices ("each GPU has the information of spins ... of a sub-lattice",
+ * PAPER.md:62), one per entry of `devices` (piece (px, py) = devices[py * gx + px]; NULL = the current device for
+ * all; several pieces may share a device).  Labeling is two-stage: inside each piece, then between
+ * pieces over the boundary sites only; label values are global site indices, the new state of a cluster comes from the
+ * Philox key of its canonical root, so bonds, labels, spins and observables are IDENTICAL to those of sw_create with
+ * the same (L, q, K, seed) -- the calls below mirror sw_init / sw_set_state / sw_sweep / sw_measure / sw_get_*, with
+ * host arrays in the layout of the whole lattice (site i = y*L + x).
+ * L % (64 gx) == 0 and L % (64 gy) == 0, gx*gy <= 64, 64 <= L <= 65536; devices that differ must have peer access
+ * (NVLink): the bond kernel reads its neighbours' boundary spins and the inter-piece merge hooks roots with
+ * system-scope atomicMin directly in the owner's memory.  Device memory is owned by the library.                  */
+typedef struct sw_super sw_super;
+int  sw_create_super(sw_super **out, uint32_t L, uint32_t q, double K, uint64_t seed,
+                     uint32_t gx, uint32_t gy, const int *devices /* [gx*gy] or NULL */);
+void sw_super_destroy(sw_super *s);
+int  sw_super_init(sw_super *s, int mode);
+int  sw_super_set_state(sw_super *s, const uint8_t *src /* host [L*L] */, uint64_t t);
+int  sw_super_sweep(sw_super *s, uint64_t n);                 /* asynchronous on the pieces' streams */
+int  sw_super_measure(sw_super *s, uint64_t *energy_bonds, uint64_t *mag_counts /* [q] */,
+                      uint64_t *n_clusters, uint64_t *largest_cluster);
+int  sw_super_get_spins(sw_super *s, uint8_t *dst /* host [L*L] */);
+int  sw_super_get_labels(sw_super *s, uint32_t *dst /* host [L*L], canonical roots = global site indices */);
+int  sw_super_get_bonds(sw_super *s, uint8_t *dst /* host [L*L], bit0 right, bit1 down */);
+int  sw_super_get_time(sw_super *s, uint64_t *t);
+int  sw_super_synchronize(sw_super *s);
+typedef struct sw_super_stats {
+    uint32_t gx, gy, piece_w, piece_h;  /* the decomposition                                                      */
+    uint32_t devices;                   /* distinct devices in use                                                */
+    uint64_t sweeps, kernel_launches, device_bytes;
+    uint64_t boundary_sites_per_piece;  /* 2 (W + H): all that stage 2 looks at ("4 N_x")             */
+    uint64_t inter_links;               /* active bonds between pieces united by stage 2, all sweeps              */
+    uint64_t inter_hops;                /* label loads of stage 2 + resolve (local or over NVLink)                */
+    uint64_t inter_retries;             /* hooks that lost the race for a root                                    */
+    uint64_t resolved_links;            /* links leaving a piece that the resolve pass re-pointed at the root     */
+} sw_super_stats;
+int  sw_super_get_stats(sw_super *s, sw_super_stats *out);
+const char *sw_super_last_error(const sw_super *s);
+
 #ifdef __cplusplus
 }
 #endif

@@ -30,6 +30,9 @@ SYMBOLS = [
     "sw_get_bonds", "sw_get_rows", "sw_get_threshold", "sw_get_time", "sw_synchronize",
     "sw_get_stats", "sw_profile_begin", "sw_profile_end", "sw_profile_series", "sw_kernel_name", "sw_last_error",
     "sw_version",
+    "sw_create_super", "sw_super_destroy", "sw_super_init", "sw_super_set_state", "sw_super_sweep", "sw_super_measure",
+    "sw_super_get_spins", "sw_super_get_labels", "sw_super_get_bonds", "sw_super_get_time", "sw_super_synchronize",
+    "sw_super_get_stats", "sw_super_last_error",
 ]
 
 
@@ -47,6 +50,13 @@ class Stats(C.Structure):
                 ("merge_links", C.c_uint64), ("merge_retries", C.c_uint64), ("merge_hops", C.c_uint64),
                 ("chase_hops", C.c_uint64), ("max_merge_depth", C.c_uint32), ("max_chase_depth", C.c_uint32),
                 ("bytes_moved", C.c_uint64)]
+
+
+class SuperStats(C.Structure):
+    _fields_ = [("gx", C.c_uint32), ("gy", C.c_uint32), ("piece_w", C.c_uint32), ("piece_h", C.c_uint32), ("devices", C.c_uint32),
+                ("sweeps", C.c_uint64), ("kernel_launches", C.c_uint64), ("device_bytes", C.c_uint64),
+                ("boundary_sites_per_piece", C.c_uint64), ("inter_links", C.c_uint64), ("inter_hops", C.c_uint64),
+                ("inter_retries", C.c_uint64), ("resolved_links", C.c_uint64)]
 
 
 def lib():
@@ -86,6 +96,19 @@ def lib():
     l.sw_kernel_name.argtypes = [vp, C.c_int]; l.sw_kernel_name.restype = C.c_char_p
     l.sw_last_error.argtypes = [vp]; l.sw_last_error.restype = C.c_char_p
     l.sw_version.argtypes = []; l.sw_version.restype = C.c_char_p
+    l.sw_create_super.argtypes = [C.POINTER(vp), C.c_uint32, C.c_uint32, C.c_double, C.c_uint64, C.c_uint32, C.c_uint32, C.POINTER(C.c_int)]
+    l.sw_super_destroy.argtypes = [vp]; l.sw_super_destroy.restype = None
+    l.sw_super_init.argtypes = [vp, C.c_int]
+    l.sw_super_set_state.argtypes = [vp, vp, C.c_uint64]
+    l.sw_super_sweep.argtypes = [vp, C.c_uint64]
+    l.sw_super_measure.argtypes = [vp, u64p, u64p, u64p, u64p]
+    l.sw_super_get_spins.argtypes = [vp, vp]
+    l.sw_super_get_labels.argtypes = [vp, vp]
+    l.sw_super_get_bonds.argtypes = [vp, vp]
+    l.sw_super_get_time.argtypes = [vp, u64p]
+    l.sw_super_synchronize.argtypes = [vp]
+    l.sw_super_get_stats.argtypes = [vp, C.POINTER(SuperStats)]
+    l.sw_super_last_error.argtypes = [vp]; l.sw_super_last_error.restype = C.c_char_p
     for name in SYMBOLS:
         getattr(l, name)                         # AttributeError here = the library is stale
     _lib = l
@@ -246,3 +269,92 @@ class SwendsenWang:
             if name and n[slot]:
                 out[name.decode()] = {"ms": float(ms[slot]), "launches": int(n[slot])}
         return out
+
+
+class SuperLattice:
+    """The gx x gy super-lattice decomposition driven from one process; same results as SwendsenWang.
+
+    `devices`: one CUDA device index per piece (row-major, piece (px, py) = devices[py * gx + px]); None = the current
+    device for every piece.  Method names follow include/sw.h without the `sw_super_` prefix."""
+
+    def __init__(self, L, q, K, seed, gx, gy, devices=None):
+        self.L, self.q, self.K, self.seed, self.gx, self.gy = int(L), int(q), float(K), int(seed), int(gx), int(gy)
+        self.N = self.L * self.L
+        self._h = C.c_void_p()
+        dev = None
+        if devices is not None:
+            if len(devices) != self.gx * self.gy:
+                raise SwError(ERR_INVALID_ARG, "sw_create_super", "one device per piece")
+            dev = (C.c_int * len(devices))(*[int(d) for d in devices])
+        rc = lib().sw_create_super(C.byref(self._h), self.L, self.q, self.K, self.seed, self.gx, self.gy, dev)
+        if rc != OK:
+            self._h = C.c_void_p()
+            raise SwError(rc, "sw_create_super")
+
+    def close(self):
+        if self._h:
+            lib().sw_super_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _chk(self, rc, what):
+        if rc != OK:
+            msg = lib().sw_super_last_error(self._h)
+            raise SwError(rc, what, msg.decode() if msg else "")
+
+    def init(self, mode):
+        self._chk(lib().sw_super_init(self._h, {"ordered": INIT_ORDERED, "random": INIT_RANDOM}.get(mode, mode)), "sw_super_init")
+
+    def set_state(self, spins, t):
+        s = np.ascontiguousarray(spins, dtype=np.uint8).reshape(-1)
+        if s.size != self.N:
+            raise SwError(ERR_INVALID_ARG, "sw_super_set_state", "wrong number of spins")
+        self._chk(lib().sw_super_set_state(self._h, s.ctypes.data, int(t)), "sw_super_set_state")
+
+    def sweep(self, n=1):
+        self._chk(lib().sw_super_sweep(self._h, int(n)), "sw_super_sweep")
+
+    def measure(self, energy=True, mag=True, clusters=True, largest=True):
+        e, nc, big = C.c_uint64(), C.c_uint64(), C.c_uint64()
+        m = (C.c_uint64 * self.q)()
+        self._chk(lib().sw_super_measure(self._h, C.byref(e) if energy else None, m if mag else None,
+                                         C.byref(nc) if clusters else None, C.byref(big) if largest else None), "sw_super_measure")
+        out = {}
+        if energy: out["energy_bonds"] = int(e.value)
+        if mag: out["mag_counts"] = [int(v) for v in m]
+        if clusters: out["n_clusters"] = int(nc.value)
+        if largest: out["largest_cluster"] = int(big.value)
+        return out
+
+    def get_spins(self):
+        out = np.empty(self.N, dtype=np.uint8)
+        self._chk(lib().sw_super_get_spins(self._h, out.ctypes.data), "sw_super_get_spins")
+        return out
+
+    def get_labels(self):
+        out = np.empty(self.N, dtype=np.uint32)
+        self._chk(lib().sw_super_get_labels(self._h, out.ctypes.data), "sw_super_get_labels")
+        return out
+
+    def get_bonds(self):
+        out = np.empty(self.N, dtype=np.uint8)
+        self._chk(lib().sw_super_get_bonds(self._h, out.ctypes.data), "sw_super_get_bonds")
+        return out
+
+    def get_time(self):
+        t = C.c_uint64()
+        self._chk(lib().sw_super_get_time(self._h, C.byref(t)), "sw_super_get_time")
+        return int(t.value)
+
+    def synchronize(self):
+        self._chk(lib().sw_super_synchronize(self._h), "sw_super_synchronize")
+
+    def stats(self):
+        s = SuperStats()
+        self._chk(lib().sw_super_get_stats(self._h, C.byref(s)), "sw_super_get_stats")
+        return {f: int(getattr(s, f)) for f, _ in SuperStats._fields_}

@@ -10,8 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsw.so")
 SOURCES = ["sw_api.cu"]
-DEPS = ["sw_api.cu", "sw_common.cuh", "sw_generic.cuh", "sw_tiled.cuh", "sw_tile_blocks.cuh", "sw_observe.cuh",
-        os.path.join("..", "..", "include", "sw.h")]
+DEPS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h"))) + [os.path.join("..", "..", "include", "sw.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=default"]

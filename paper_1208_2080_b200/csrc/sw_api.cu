@@ -729,3 +729,6 @@ const char *sw_kernel_name(sw_ctx *c, int slot)
 const char *sw_last_error(const sw_ctx *c) { return c ? c->err.c_str() : "null context"; }
 
 }  // extern "C"
+
+// the super-lattice decomposition: same translation unit, its own context type
+#include "sw_super.cuh"
