@@ -218,6 +218,23 @@ typedef struct sw_super_stats {
 int  sw_super_get_stats(sw_super *s, sw_super_stats *out);
 const char *sw_super_last_error(const sw_super *s);
 
+/* One process per GPU (the launch the paper uses: one MPI rank per GPU).  Every rank creates a context that
+ * OWNS one piece (on its current device) and learns where the other pieces are through CUDA IPC: each rank exports the
+ * 64-byte handle of its piece, the ranks exchange them (torch.distributed all_gather in the Python binding) and import
+ * the others'.  A sweep is three phases (0: stage 1 inside the piece, 1: stage 2 between pieces, 2: resolve + flatten +
+ * flip); the caller calls sw_super_synchronize and a barrier of the process group after each phase -- that barrier is all
+ * that is left of the paper's per-round flag exchange.  sw_super_init / _set_state / _get_* act on the
+ * local piece (host arrays keep the layout of the whole lattice; only the local piece's part is read / written).
+ * A measurement is three phases as well (0: zero, 1: count, 2: maxima and the local partial row [3+q]: all columns are
+ * sums over the ranks except column 2, largest_cluster, which is a maximum).                                           */
+#define SW_IPC_HANDLE_BYTES 64
+int  sw_create_super_rank(sw_super **out, uint32_t L, uint32_t q, double K, uint64_t seed,
+                          uint32_t gx, uint32_t gy, uint32_t my_piece);
+int  sw_super_ipc_export(sw_super *s, void *handle_out /* host [SW_IPC_HANDLE_BYTES] */);
+int  sw_super_ipc_import(sw_super *s, uint32_t piece, const void *handle /* host [SW_IPC_HANDLE_BYTES] */);
+int  sw_super_phase(sw_super *s, int phase /* 0, 1, 2; phase 2 advances the sweep counter */);
+int  sw_super_measure_phase(sw_super *s, int phase, uint32_t what /* SW_OBS_* */, uint64_t *part /* host [3+q], phase 2 */);
+
 #ifdef __cplusplus
 }
 #endif

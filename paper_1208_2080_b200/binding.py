@@ -33,6 +33,7 @@ SYMBOLS = [
     "sw_create_super", "sw_super_destroy", "sw_super_init", "sw_super_set_state", "sw_super_sweep", "sw_super_measure",
     "sw_super_get_spins", "sw_super_get_labels", "sw_super_get_bonds", "sw_super_get_time", "sw_super_synchronize",
     "sw_super_get_stats", "sw_super_last_error",
+    "sw_create_super_rank", "sw_super_ipc_export", "sw_super_ipc_import", "sw_super_phase", "sw_super_measure_phase",
 ]
 
 

@@ -242,6 +242,8 @@ using sw::Dom;
 using sw::Params;
 
 struct Piece {
+    bool local = true;              // false: another process owns it; only the peer pointers (opened through CUDA IPC) are known
+    void *ipc_base = nullptr;       // what cudaIpcOpenMemHandle returned for a remote piece
     int device = 0;
     uint32_t px = 0, py = 0;
     cudaStream_t stream = nullptr;
@@ -267,6 +269,7 @@ struct sw_super {
     uint64_t N = 0, seed = 0, T = 0, t = 0, draws_t = ~0ull;
     double K = 0;
     bool have_spins = false, have_labels = false;
+    int rank_piece = -1;            // >= 0: one process per GPU, this process owns that piece only (sw_create_super_rank)
     uint64_t launches = 0, sweeps = 0;
     std::vector<Piece> pieces;
     sw::SuperGeo geo{};
@@ -311,13 +314,62 @@ uint32_t down_of(const sw_super *s, uint32_t d) { const uint32_t px = d % s->gx,
 
 int grid_cap(uint64_t items, int threads) { return (int)std::max<uint64_t>(1, std::min<uint64_t>((items + threads - 1) / threads, 148 * 16)); }
 
+// byte offsets of a piece's arrays inside its one allocation: the same for every piece, so a process that opened
+// another piece's allocation through CUDA IPC knows where its spins, labels and edge records are
+struct PieceLayout { size_t spins, bonds, labels, rootbits, border, edges, tc, draws, row, flag, cnt, stage, stage_bytes, sizes, total; };
+
+PieceLayout piece_layout(const sw_super *s)
+{
+    const uint64_t Np = (uint64_t)s->W * s->H, tiles = Np / sw::kTileSites;
+    PieceLayout o{};
+    size_t off = 0;
+    auto carve = [&](size_t bytes) { const size_t at = off; off = swh::align_up(off + bytes); return at; };
+    o.spins = carve(Np); o.bonds = carve((Np / 16) * 4); o.labels = carve(Np * 4); o.rootbits = carve((Np / 16) * 2);
+    o.border = carve(tiles * sizeof(sw::TileBorder)); o.edges = carve(tiles * sizeof(sw::TileEdges));
+    o.tc = carve(tiles * (sw::kFlipThreads / 32) * 4); o.draws = carve((Np / 32) * sizeof(uint2));
+    o.row = carve((3 + (size_t)s->q) * 8); o.flag = carve(4); o.cnt = carve(sizeof(sw::SuperCounters));
+    o.stage_bytes = (size_t)std::min<uint64_t>(Np, std::max<uint64_t>(s->W, 32ull << 20));
+    o.stage = carve(o.stage_bytes);
+    o.sizes = carve(Np * 4);                                 // cluster-size scratch: other pieces add to it (sw_super_measure of the largest cluster)
+    o.total = off;
+    return o;
+}
+
+void set_piece_pointers(Piece &p, uint8_t *base, const PieceLayout &o)
+{
+    p.ws = base; p.ws_bytes = o.total; p.stage_bytes = o.stage_bytes;
+    p.spins = base + o.spins; p.bonds = (uint32_t *)(base + o.bonds); p.labels = (uint32_t *)(base + o.labels);
+    p.rootbits = (uint16_t *)(base + o.rootbits); p.border = (sw::TileBorder *)(base + o.border); p.edges = (sw::TileEdges *)(base + o.edges);
+    p.tile_clusters = (uint32_t *)(base + o.tc); p.draws = (uint2 *)(base + o.draws); p.row = (unsigned long long *)(base + o.row);
+    p.flag = (uint32_t *)(base + o.flag); p.counters = (sw::SuperCounters *)(base + o.cnt); p.stage = base + o.stage;
+    p.sizes = (uint32_t *)(base + o.sizes);
+}
+
+// (re)build the tables the kernels take by value: every piece's labels / edge records / size scratch, the neighbours' spins
+void refresh_geo(sw_super *s)
+{
+    const uint32_t n = (uint32_t)s->pieces.size();
+    s->geo.Lg = s->L; s->geo.log2Lg = swh::log2_exact(s->L); s->geo.gx = s->gx; s->geo.gy = s->gy; s->geo.W = s->W; s->geo.H = s->H;
+    for (uint32_t d = 0; d < n; ++d) {
+        Piece &p = s->pieces[d];
+        s->geo.labels[d] = p.labels; s->geo.edges[d] = p.edges; s->geo.sizes[d] = p.sizes;
+        const Piece &r = s->pieces[right_of(s, d)], &dn = s->pieces[down_of(s, d)];
+        p.dom.W = s->W; p.dom.H = s->H; p.dom.Lg = s->L; p.dom.log2Lg = s->geo.log2Lg;
+        p.dom.ox = p.px * s->W; p.dom.oy = p.py * s->H;
+        p.dom.right = r.spins; p.dom.down = dn.spins; p.dom.right_W = s->W; p.dom.me = d;
+    }
+}
+
 void destroy_pieces(sw_super *s)
 {
     DevSwitch sw_;
     for (auto &p : s->pieces) {
+        if (!p.local) {
+            if (p.ipc_base) cudaIpcCloseMemHandle(p.ipc_base);
+            continue;
+        }
         sw_.to(p.device);
         if (p.stream) cudaStreamSynchronize(p.stream);
-        if (p.sizes) cudaFree(p.sizes);
         if (p.ws) cudaFree(p.ws);
         if (p.ev_stage1) cudaEventDestroy(p.ev_stage1);
         if (p.ev_stage2) cudaEventDestroy(p.ev_stage2);
@@ -327,55 +379,70 @@ void destroy_pieces(sw_super *s)
     s->pieces.clear();
 }
 
-// one sweep: stage 1 on every piece, stage 2, resolve, flatten + flip; all asynchronous, ordered by events
-int super_sweep_once(sw_super *s, bool count_clusters)
+// The three phases of a sweep.  In one process (all pieces local) they are ordered by events: a phase of a piece waits for
+// the previous phase of EVERY piece.  With one process per GPU (rank mode) the caller puts a barrier of the process group
+// between the phases (after sw_super_synchronize) and the event waits fall away.
+//   phase 0  stage 1: bonds + tile-local labels + tile-border merge inside the piece
+//   phase 1  stage 2: union over the bonds between pieces (boundary sites only)
+//   phase 2  resolve, flatten to the canonical root, flip
+int super_phase(sw_super *s, int phase, bool count_clusters)
 {
     DevSwitch sw_;
     const Params P = piece_params(s, s->t);
     const uint32_t n = (uint32_t)s->pieces.size();
     const dim3 tgrid(s->W / sw::kTile, s->H / sw::kTile);
     const uint32_t tiles = tgrid.x * tgrid.y;
-    for (uint32_t d = 0; d < n; ++d) {                      // stage 1 (needs the neighbours' spins of the previous flip)
+    for (uint32_t d = 0; d < n; ++d) {
         Piece &p = s->pieces[d];
+        if (!p.local) continue;
         sw_.to(p.device);
-        // the right / lower neighbour's new spins must be written, and nobody may still be reading my labels of the last
-        // sweep (the resolve pass of ANY piece can follow a link into my piece): wait for every piece's last flip
-        for (uint32_t o = 0; o < n; ++o) if (o != d) SS_CUDA(s, cudaStreamWaitEvent(p.stream, s->pieces[o].ev_flip, 0));
-        if (s->draws_t != s->t) { sw::k_draws_super<<<tgrid, 256, 0, p.stream>>>(p.draws, P, p.dom); s->launches += 1; }
-        sw::k_tile_blocks_super<<<tgrid, sw::kBlkThreads, 0, p.stream>>>(p.spins, p.bonds, p.labels, p.rootbits, p.border, p.edges, p.draws, P, p.dom);
-        sw::k_tile_merge_super<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, p.stream>>>(p.labels, p.border, p.edges, P, p.dom, tiles);
-        SS_CUDA(s, cudaEventRecord(p.ev_stage1, p.stream));
-        s->launches += 2;
-    }
-    for (uint32_t d = 0; d < n; ++d) {                      // stage 2: every piece's stage 1 must be complete
-        Piece &p = s->pieces[d];
-        sw_.to(p.device);
-        for (uint32_t o = 0; o < n; ++o) if (o != d) SS_CUDA(s, cudaStreamWaitEvent(p.stream, s->pieces[o].ev_stage1, 0));
-        sw::k_super_merge<<<(s->W + s->H + 127) / 128, 128, 0, p.stream>>>(s->geo, d, right_of(s, d), down_of(s, d), p.border, p.counters);
-        SS_CUDA(s, cudaEventRecord(p.ev_stage2, p.stream));
-        s->launches += 1;
-    }
-    for (uint32_t d = 0; d < n; ++d) {                      // resolve + flatten + flip: every piece's stage 2 must be complete
-        Piece &p = s->pieces[d];
-        sw_.to(p.device);
-        for (uint32_t o = 0; o < n; ++o) if (o != d) SS_CUDA(s, cudaStreamWaitEvent(p.stream, s->pieces[o].ev_stage2, 0));
-        sw::k_super_resolve<<<(2 * (s->W + s->H) + 127) / 128, 128, 0, p.stream>>>(s->geo, p.dom, p.counters);
-        auto flip = count_clusters ? sw::k_tile_flip_super<true, true, true> : sw::k_tile_flip_super<true, true, false>;
-        flip<<<tgrid, sw::kFlipThreads, 0, p.stream>>>(p.labels, p.rootbits, p.spins, P, p.dom, p.tile_clusters, p.draws);
-        SS_CUDA(s, cudaEventRecord(p.ev_flip, p.stream));
-        s->launches += 2;
+        for (uint32_t o = 0; o < n; ++o) {
+            const Piece &other = s->pieces[o];
+            if (o == d || !other.local) continue;
+            // phase 0 waits for every piece's last flip: the neighbours' new spins must be written, and nobody may still be
+            // following links into my labels of the last sweep (the resolve pass of ANY piece can)
+            SS_CUDA(s, cudaStreamWaitEvent(p.stream, phase == 0 ? other.ev_flip : phase == 1 ? other.ev_stage1 : other.ev_stage2, 0));
+        }
+        if (phase == 0) {
+            if (s->draws_t != s->t) { sw::k_draws_super<<<tgrid, 256, 0, p.stream>>>(p.draws, P, p.dom); s->launches += 1; }
+            sw::k_tile_blocks_super<<<tgrid, sw::kBlkThreads, 0, p.stream>>>(p.spins, p.bonds, p.labels, p.rootbits, p.border, p.edges, p.draws, P, p.dom);
+            sw::k_tile_merge_super<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, p.stream>>>(p.labels, p.border, p.edges, P, p.dom, tiles);
+            SS_CUDA(s, cudaEventRecord(p.ev_stage1, p.stream));
+            s->launches += 2;
+        } else if (phase == 1) {
+            sw::k_super_merge<<<(s->W + s->H + 127) / 128, 128, 0, p.stream>>>(s->geo, d, right_of(s, d), down_of(s, d), p.border, p.counters);
+            SS_CUDA(s, cudaEventRecord(p.ev_stage2, p.stream));
+            s->launches += 1;
+        } else {
+            sw::k_super_resolve<<<(2 * (s->W + s->H) + 127) / 128, 128, 0, p.stream>>>(s->geo, p.dom, p.counters);
+            auto flip = count_clusters ? sw::k_tile_flip_super<true, true, true> : sw::k_tile_flip_super<true, true, false>;
+            flip<<<tgrid, sw::kFlipThreads, 0, p.stream>>>(p.labels, p.rootbits, p.spins, P, p.dom, p.tile_clusters, p.draws);
+            SS_CUDA(s, cudaEventRecord(p.ev_flip, p.stream));
+            s->launches += 2;
+        }
     }
     SS_CUDA(s, cudaGetLastError());
-    s->draws_t = s->t + 1;
-    s->t += 1; s->sweeps += 1;
-    s->have_labels = true;
+    if (phase == 2) {
+        s->draws_t = s->t + 1;
+        s->t += 1; s->sweeps += 1;
+        s->have_labels = true;
+    }
+    return SW_OK;
+}
+
+int super_sweep_once(sw_super *s, bool count_clusters)
+{
+    for (int phase = 0; phase < 3; ++phase) {
+        const int rc = super_phase(s, phase, count_clusters);
+        if (rc != SW_OK) return rc;
+    }
     return SW_OK;
 }
 
 int sync_all(sw_super *s)
 {
     DevSwitch sw_;
-    for (auto &p : s->pieces) { sw_.to(p.device); SS_CUDA(s, cudaStreamSynchronize(p.stream)); }
+    for (auto &p : s->pieces) { if (!p.local) continue; sw_.to(p.device); SS_CUDA(s, cudaStreamSynchronize(p.stream)); }
     return SW_OK;
 }
 
@@ -383,7 +450,7 @@ int sync_all(sw_super *s)
 int mark_spins_ready(sw_super *s)
 {
     DevSwitch sw_;
-    for (auto &p : s->pieces) { sw_.to(p.device); SS_CUDA(s, cudaEventRecord(p.ev_flip, p.stream)); }
+    for (auto &p : s->pieces) { if (!p.local) continue; sw_.to(p.device); SS_CUDA(s, cudaEventRecord(p.ev_flip, p.stream)); }
     return SW_OK;
 }
 
@@ -391,19 +458,22 @@ int mark_spins_ready(sw_super *s)
 
 extern "C" {
 
-int sw_create_super(sw_super **out, uint32_t L, uint32_t q, double K, uint64_t seed, uint32_t gx, uint32_t gy, const int *devices)
+static int create_super_common(sw_super **out, uint32_t L, uint32_t q, double K, uint64_t seed, uint32_t gx, uint32_t gy,
+                               const int *devices, int rank_piece)
 {
     if (!out) return SW_ERR_INVALID_ARG;
     *out = nullptr;
     uint64_t T = 0;
     if (L < 64 || L > 65536 || q < 2 || q > 255 || !swh::host_threshold(K, &T)) return SW_ERR_INVALID_ARG;
     if (gx < 1 || gy < 1 || gx * gy > (uint32_t)sw::kMaxPieces || L % (gx * sw::kTile) || L % (gy * sw::kTile)) return SW_ERR_INVALID_ARG;
+    if (rank_piece >= (int)(gx * gy)) return SW_ERR_INVALID_ARG;
     sw_super *s = new (std::nothrow) sw_super();
     if (!s) return SW_ERR_OOM;
     s->L = L; s->q = q; s->K = K; s->seed = seed; s->T = T; s->gx = gx; s->gy = gy;
     s->W = L / gx; s->H = L / gy; s->N = (uint64_t)L * L;
+    s->rank_piece = rank_piece;
     const uint32_t n = gx * gy;
-    const uint64_t Np = (uint64_t)s->W * s->H, tiles = Np / sw::kTileSites;
+    const PieceLayout lay = piece_layout(s);
     DevSwitch sw_;
     int cur = 0, count = 0;
     if (cudaGetDevice(&cur) != cudaSuccess || cudaGetDeviceCount(&count) != cudaSuccess) { delete s; return SW_ERR_CUDA; }
@@ -411,24 +481,15 @@ int sw_create_super(sw_super **out, uint32_t L, uint32_t q, double K, uint64_t s
     int rc = SW_OK;
     for (uint32_t d = 0; d < n && rc == SW_OK; ++d) {
         Piece &p = s->pieces[d];
-        p.device = devices ? devices[d] : cur;
         p.px = d % gx; p.py = d / gx;
+        p.local = rank_piece < 0 || (int)d == rank_piece;
+        if (!p.local) continue;                              // its pointers arrive through sw_super_ipc_import
+        p.device = (devices && rank_piece < 0) ? devices[d] : cur;
         if (p.device < 0 || p.device >= count) { rc = SW_ERR_INVALID_ARG; break; }
         sw_.to(p.device);
-        size_t off = 0;
-        auto carve = [&](size_t bytes) { const size_t at = off; off = swh::align_up(off + bytes); return at; };
-        const size_t o_spins = carve(Np), o_bonds = carve((Np / 16) * 4), o_labels = carve(Np * 4), o_rootbits = carve((Np / 16) * 2);
-        const size_t o_border = carve(tiles * sizeof(sw::TileBorder)), o_edges = carve(tiles * sizeof(sw::TileEdges));
-        const size_t o_tc = carve(tiles * (sw::kFlipThreads / 32) * 4), o_draws = carve((Np / 32) * sizeof(uint2));
-        const size_t o_row = carve((3 + (size_t)q) * 8), o_flag = carve(4), o_cnt = carve(sizeof(sw::SuperCounters));
-        p.stage_bytes = (size_t)std::min<uint64_t>(Np, std::max<uint64_t>(s->W, 32ull << 20));
-        const size_t o_stage = carve(p.stage_bytes);
-        p.ws_bytes = off;
-        if (cudaMalloc(&p.ws, p.ws_bytes) != cudaSuccess) { cudaGetLastError(); rc = SW_ERR_OOM; break; }
-        p.spins = p.ws + o_spins; p.bonds = (uint32_t *)(p.ws + o_bonds); p.labels = (uint32_t *)(p.ws + o_labels);
-        p.rootbits = (uint16_t *)(p.ws + o_rootbits); p.border = (sw::TileBorder *)(p.ws + o_border); p.edges = (sw::TileEdges *)(p.ws + o_edges);
-        p.tile_clusters = (uint32_t *)(p.ws + o_tc); p.draws = (uint2 *)(p.ws + o_draws); p.row = (unsigned long long *)(p.ws + o_row);
-        p.flag = (uint32_t *)(p.ws + o_flag); p.counters = (sw::SuperCounters *)(p.ws + o_cnt); p.stage = p.ws + o_stage;
+        uint8_t *base = nullptr;
+        if (cudaMalloc(&base, lay.total) != cudaSuccess) { cudaGetLastError(); rc = SW_ERR_OOM; break; }
+        set_piece_pointers(p, base, lay);
         if (cudaStreamCreateWithFlags(&p.stream, cudaStreamNonBlocking) != cudaSuccess ||
             cudaEventCreateWithFlags(&p.ev_stage1, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&p.ev_stage2, cudaEventDisableTiming) != cudaSuccess ||
@@ -436,30 +497,71 @@ int sw_create_super(sw_super **out, uint32_t L, uint32_t q, double K, uint64_t s
             cudaMemsetAsync(p.counters, 0, sizeof(sw::SuperCounters), p.stream) != cudaSuccess) { cudaGetLastError(); rc = SW_ERR_CUDA; break; }
     }
     // peer access between the devices in use (NVLink P2P); pieces on one device need none
-    for (uint32_t a = 0; a < n && rc == SW_OK; ++a)
+    for (uint32_t a = 0; a < n && rc == SW_OK && rank_piece < 0; ++a)
         for (uint32_t b = 0; b < n && rc == SW_OK; ++b) {
             const int da = s->pieces[a].device, db = s->pieces[b].device;
             if (da == db) continue;
             int can = 0;
             cudaDeviceCanAccessPeer(&can, da, db);
-            if (!can) { s->err = "no peer access between the devices of two pieces"; rc = SW_ERR_CUDA; break; }
+            if (!can) { rc = SW_ERR_CUDA; break; }
             sw_.to(da);
             const cudaError_t e = cudaDeviceEnablePeerAccess(db, 0);
             if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) rc = SW_ERR_CUDA;
             cudaGetLastError();
         }
     if (rc != SW_OK) { destroy_pieces(s); delete s; return rc; }
-    s->geo.Lg = L; s->geo.log2Lg = swh::log2_exact(L); s->geo.gx = gx; s->geo.gy = gy; s->geo.W = s->W; s->geo.H = s->H;
-    for (uint32_t d = 0; d < n; ++d) {
-        Piece &p = s->pieces[d];
-        s->geo.labels[d] = p.labels; s->geo.edges[d] = p.edges; s->geo.sizes[d] = nullptr;
-        const Piece &r = s->pieces[right_of(s, d)], &dn = s->pieces[down_of(s, d)];
-        p.dom.W = s->W; p.dom.H = s->H; p.dom.Lg = L; p.dom.log2Lg = s->geo.log2Lg;
-        p.dom.ox = p.px * s->W; p.dom.oy = p.py * s->H;
-        p.dom.right = r.spins; p.dom.down = dn.spins; p.dom.right_W = s->W; p.dom.me = d;
-    }
+    refresh_geo(s);
     *out = s;
     return SW_OK;
+}
+
+int sw_create_super(sw_super **out, uint32_t L, uint32_t q, double K, uint64_t seed, uint32_t gx, uint32_t gy, const int *devices)
+{
+    return create_super_common(out, L, q, K, seed, gx, gy, devices, -1);
+}
+
+int sw_create_super_rank(sw_super **out, uint32_t L, uint32_t q, double K, uint64_t seed, uint32_t gx, uint32_t gy, uint32_t my_piece)
+{
+    if (my_piece >= gx * gy) return SW_ERR_INVALID_ARG;
+    return create_super_common(out, L, q, K, seed, gx, gy, nullptr, (int)my_piece);
+}
+
+int sw_super_ipc_export(sw_super *s, void *handle_out)
+{
+    if (!s || !handle_out || s->rank_piece < 0) return sfail(s, SW_ERR_INVALID_ARG, "sw_super_ipc_export: not a rank context");
+    static_assert(sizeof(cudaIpcMemHandle_t) == SW_IPC_HANDLE_BYTES, "handle size");
+    DevSwitch sw_;
+    Piece &p = s->pieces[s->rank_piece];
+    sw_.to(p.device);
+    SS_CUDA(s, cudaIpcGetMemHandle((cudaIpcMemHandle_t *)handle_out, p.ws));
+    return SW_OK;
+}
+
+int sw_super_ipc_import(sw_super *s, uint32_t piece, const void *handle)
+{
+    if (!s || !handle || s->rank_piece < 0 || piece >= s->pieces.size() || (int)piece == s->rank_piece)
+        return sfail(s, SW_ERR_INVALID_ARG, "sw_super_ipc_import: bad argument");
+    Piece &p = s->pieces[piece];
+    if (p.ipc_base) return sfail(s, SW_ERR_STATE, "sw_super_ipc_import: piece already imported");
+    DevSwitch sw_;
+    sw_.to(s->pieces[s->rank_piece].device);
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle, sizeof(h));
+    void *base = nullptr;
+    SS_CUDA(s, cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess));
+    p.ipc_base = base;
+    set_piece_pointers(p, (uint8_t *)base, piece_layout(s));
+    refresh_geo(s);
+    return SW_OK;
+}
+
+int sw_super_phase(sw_super *s, int phase)
+{
+    if (!s || phase < 0 || phase > 2) return SW_ERR_INVALID_ARG;
+    if (!s->have_spins) return sfail(s, SW_ERR_STATE, "sw_super_phase: no spins");
+    if (s->t + 1 > 0x100000000ull) return sfail(s, SW_ERR_STATE, "sw_super_phase: sweep counter would pass 2^32");
+    for (auto &p : s->pieces) if (!p.spins) return sfail(s, SW_ERR_STATE, "sw_super_phase: a piece has not been imported");
+    return super_phase(s, phase, true);
 }
 
 void sw_super_destroy(sw_super *s)
@@ -476,6 +578,7 @@ int sw_super_init(sw_super *s, int mode)
     DevSwitch sw_;
     const Params P = piece_params(s, 0);
     for (auto &p : s->pieces) {
+        if (!p.local) continue;
         sw_.to(p.device);
         if (mode == SW_INIT_ORDERED) SS_CUDA(s, cudaMemsetAsync(p.spins, 0, (size_t)s->W * s->H, p.stream));
         else { sw::k_init_random_super<<<grid_cap((uint64_t)s->W * s->H, 256), 256, 0, p.stream>>>(p.spins, P, p.dom); s->launches += 1; }
@@ -491,6 +594,7 @@ int sw_super_set_state(sw_super *s, const uint8_t *src, uint64_t t)
     DevSwitch sw_;
     Params P = piece_params(s, 0);
     for (auto &p : s->pieces) {
+        if (!p.local) continue;
         sw_.to(p.device);
         const uint8_t *from = src + (uint64_t)p.dom.oy * s->L + p.dom.ox;
         SS_CUDA(s, cudaMemcpy2DAsync(p.spins, s->W, from, s->L, s->W, s->H, cudaMemcpyHostToDevice, p.stream));
@@ -500,6 +604,7 @@ int sw_super_set_state(sw_super *s, const uint8_t *src, uint64_t t)
     }
     bool bad = false;
     for (auto &p : s->pieces) {
+        if (!p.local) continue;
         sw_.to(p.device);
         uint32_t f = 0;
         SS_CUDA(s, cudaMemcpyAsync(&f, p.flag, 4, cudaMemcpyDeviceToHost, p.stream));
@@ -515,6 +620,7 @@ int sw_super_set_state(sw_super *s, const uint8_t *src, uint64_t t)
 int sw_super_sweep(sw_super *s, uint64_t n)
 {
     if (!s) return SW_ERR_INVALID_ARG;
+    if (s->rank_piece >= 0) return sfail(s, SW_ERR_STATE, "sw_super_sweep: one process per GPU: drive the sweep with sw_super_phase and a barrier between the phases");
     if (!s->have_spins) return sfail(s, SW_ERR_STATE, "sw_super_sweep: no spins (call sw_super_init or sw_super_set_state)");
     if (s->t + n > 0x100000000ull) return sfail(s, SW_ERR_STATE, "sw_super_sweep: sweep counter would pass 2^32");
     for (uint64_t k = 0; k < n; ++k) {
@@ -524,58 +630,66 @@ int sw_super_sweep(sw_super *s, uint64_t n)
     return SW_OK;
 }
 
-int sw_super_measure(sw_super *s, uint64_t *energy_bonds, uint64_t *mag_counts, uint64_t *n_clusters, uint64_t *largest_cluster)
+// The three phases of a measurement, over the local pieces (a barrier between them in rank mode, a sync here otherwise):
+//   0  zero the rows and, for the largest cluster, the size counters
+//   1  equal pairs + histogram, cluster count, sizes[owner(root)] += members (into other pieces' memory too)
+//   2  maximum of the local size counters; the local partial row comes back in `part` (sum columns; column 2 is a maximum)
+static int measure_phase(sw_super *s, int phase, uint32_t what, uint64_t *part)
 {
-    if (!s) return SW_ERR_INVALID_ARG;
-    if (!s->have_spins) return sfail(s, SW_ERR_STATE, "sw_super_measure: no spins");
     DevSwitch sw_;
     const Params P = piece_params(s, s->t);
     const uint64_t Np = (uint64_t)s->W * s->H;
     const uint32_t n = (uint32_t)s->pieces.size();
-    const bool cl = s->have_labels && (n_clusters || largest_cluster), big = s->have_labels && largest_cluster;
-    const uint32_t want = (energy_bonds ? 1u : 0u) | (mag_counts ? 2u : 0u);
-    int rc = sync_all(s);                                     // the spins of all pieces are final
-    if (rc != SW_OK) return rc;
-    if (big) {
-        for (uint32_t d = 0; d < n; ++d) {
-            Piece &p = s->pieces[d];
-            sw_.to(p.device);
-            if (!p.sizes) { SS_CUDA(s, cudaMalloc(&p.sizes, Np * 4)); s->geo.sizes[d] = p.sizes; }
-            SS_CUDA(s, cudaMemsetAsync(p.sizes, 0, Np * 4, p.stream));
-        }
-        rc = sync_all(s);
-        if (rc != SW_OK) return rc;
-    }
+    const bool cl = s->have_labels && (what & (SW_OBS_CLUSTERS | SW_OBS_LARGEST)), big = s->have_labels && (what & SW_OBS_LARGEST);
+    const uint32_t want = what & 3u;
+    const size_t cols = 3 + (size_t)s->q;
+    if (phase == 2 && part) for (size_t k = 0; k < cols; ++k) part[k] = 0;
     for (uint32_t d = 0; d < n; ++d) {
         Piece &p = s->pieces[d];
+        if (!p.local) continue;
         sw_.to(p.device);
-        SS_CUDA(s, cudaMemsetAsync(p.row, 0, (3 + (size_t)s->q) * 8, p.stream));
-        if (want) { sw::k_super_observe<<<grid_cap(Np, sw::kObsThreads), sw::kObsThreads, 0, p.stream>>>(p.spins, P, p.dom, want, p.row); s->launches += 1; }
-        if (cl) {
-            const uint32_t entries = (uint32_t)(Np / sw::kTileSites) * (sw::kFlipThreads / 32);
-            sw::k_sum_tile_clusters<<<grid_cap(entries, sw::kObsThreads), sw::kObsThreads, 0, p.stream>>>(p.tile_clusters, entries, p.row);
-            s->launches += 1;
-        }
-        if (big) { sw::k_super_sizes<<<grid_cap(Np / 16, 256), 256, 0, p.stream>>>(s->geo, d); s->launches += 1; }
-    }
-    if (big) {
-        rc = sync_all(s);                                     // all counts are in
-        if (rc != SW_OK) return rc;
-        for (uint32_t d = 0; d < n; ++d) {
-            Piece &p = s->pieces[d];
-            sw_.to(p.device);
-            sw::k_max_size<<<grid_cap(Np, 256), 256, 0, p.stream>>>(p.sizes, P, p.row);
-            s->launches += 1;
+        if (phase == 0) {
+            SS_CUDA(s, cudaMemsetAsync(p.row, 0, cols * 8, p.stream));
+            if (big) SS_CUDA(s, cudaMemsetAsync(p.sizes, 0, Np * 4, p.stream));
+        } else if (phase == 1) {
+            if (want) { sw::k_super_observe<<<grid_cap(Np, sw::kObsThreads), sw::kObsThreads, 0, p.stream>>>(p.spins, P, p.dom, want, p.row); s->launches += 1; }
+            if (cl) {
+                const uint32_t entries = (uint32_t)(Np / sw::kTileSites) * (sw::kFlipThreads / 32);
+                sw::k_sum_tile_clusters<<<grid_cap(entries, sw::kObsThreads), sw::kObsThreads, 0, p.stream>>>(p.tile_clusters, entries, p.row);
+                s->launches += 1;
+            }
+            if (big) { sw::k_super_sizes<<<grid_cap(Np / 16, 256), 256, 0, p.stream>>>(s->geo, d); s->launches += 1; }
+        } else {
+            if (big) { sw::k_max_size<<<grid_cap(Np, 256), 256, 0, p.stream>>>(p.sizes, P, p.row); s->launches += 1; }
+            std::vector<uint64_t> row(cols);
+            SS_CUDA(s, cudaMemcpyAsync(row.data(), p.row, cols * 8, cudaMemcpyDeviceToHost, p.stream));
+            SS_CUDA(s, cudaStreamSynchronize(p.stream));
+            if (part) for (size_t k = 0; k < cols; ++k) part[k] = (k == 2) ? std::max(part[k], row[k]) : part[k] + row[k];
         }
     }
     SS_CUDA(s, cudaGetLastError());
-    std::vector<uint64_t> total(3 + s->q, 0), row(3 + s->q);
-    for (auto &p : s->pieces) {
-        sw_.to(p.device);
-        SS_CUDA(s, cudaMemcpyAsync(row.data(), p.row, row.size() * 8, cudaMemcpyDeviceToHost, p.stream));
-        SS_CUDA(s, cudaStreamSynchronize(p.stream));
-        for (size_t k = 0; k < row.size(); ++k) total[k] = (k == 2) ? std::max(total[k], row[k]) : total[k] + row[k];
-    }
+    return sync_all(s);
+}
+
+int sw_super_measure_phase(sw_super *s, int phase, uint32_t what, uint64_t *part)
+{
+    if (!s || phase < 0 || phase > 2 || (what & ~(uint32_t)SW_OBS_ALL) || (phase == 2 && !part)) return SW_ERR_INVALID_ARG;
+    if (!s->have_spins) return sfail(s, SW_ERR_STATE, "sw_super_measure_phase: no spins");
+    for (auto &p : s->pieces) if (!p.spins) return sfail(s, SW_ERR_STATE, "sw_super_measure_phase: a piece has not been imported");
+    return measure_phase(s, phase, what, part);
+}
+
+int sw_super_measure(sw_super *s, uint64_t *energy_bonds, uint64_t *mag_counts, uint64_t *n_clusters, uint64_t *largest_cluster)
+{
+    if (!s) return SW_ERR_INVALID_ARG;
+    if (s->rank_piece >= 0) return sfail(s, SW_ERR_STATE, "sw_super_measure: one process per GPU: use sw_super_measure_phase with a barrier between the phases");
+    if (!s->have_spins) return sfail(s, SW_ERR_STATE, "sw_super_measure: no spins");
+    const uint32_t what = (energy_bonds ? SW_OBS_ENERGY : 0u) | (mag_counts ? SW_OBS_MAG : 0u) | (n_clusters ? SW_OBS_CLUSTERS : 0u) |
+                          (largest_cluster ? SW_OBS_LARGEST : 0u);
+    std::vector<uint64_t> total(3 + s->q, 0);
+    int rc = sync_all(s);                                     // the spins of all pieces are final
+    for (int phase = 0; phase < 3 && rc == SW_OK; ++phase) rc = measure_phase(s, phase, what, total.data());
+    if (rc != SW_OK) return rc;
     if (total[1] == 1) total[2] = s->N;                       // a uint32 size counter wraps only when one cluster holds 2^32 sites
     if (energy_bonds) *energy_bonds = total[0];
     if (n_clusters) *n_clusters = s->have_labels ? total[1] : 0;
@@ -590,6 +704,7 @@ static int super_get(sw_super *s, int what, void *dst)
     if (what == 0 ? !s->have_spins : !s->have_labels) return sfail(s, SW_ERR_STATE, what == 0 ? "no spins" : "no sweep since sw_super_init");
     DevSwitch sw_;
     for (auto &p : s->pieces) {
+        if (!p.local) continue;                              // rank mode: only my piece's part of dst is written
         sw_.to(p.device);
         const uint64_t first = (uint64_t)p.dom.oy * s->L + p.dom.ox;
         if (what == 0) {
@@ -633,12 +748,13 @@ int sw_super_get_stats(sw_super *s, sw_super_stats *out)
     out->boundary_sites_per_piece = 2ull * (s->W + s->H);
     std::vector<int> seen;
     for (auto &p : s->pieces) {
+        if (!p.local) continue;
         sw_.to(p.device);
         sw::SuperCounters c;
         SS_CUDA(s, cudaMemcpyAsync(&c, p.counters, sizeof(c), cudaMemcpyDeviceToHost, p.stream));
         SS_CUDA(s, cudaStreamSynchronize(p.stream));
         out->inter_links += c.links; out->inter_hops += c.hops; out->inter_retries += c.retries; out->resolved_links += c.resolved;
-        out->device_bytes += p.ws_bytes + (p.sizes ? (uint64_t)s->W * s->H * 4 : 0);
+        out->device_bytes += p.ws_bytes;
         if (std::find(seen.begin(), seen.end(), p.device) == seen.end()) seen.push_back(p.device);
     }
     out->devices = (uint32_t)seen.size();
