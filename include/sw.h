@@ -119,6 +119,12 @@ int sw_sweep(sw_ctx *ctx, uint64_t n);
 int sw_measure(sw_ctx *ctx, uint64_t *energy_bonds, uint64_t *mag_counts,
                uint64_t *n_clusters, uint64_t *largest_cluster);
 
+/* Cluster statistics of the LAST sweep with the second moment of the size distribution: sum_sq[0] + 2^64 sum_sq[1] =
+ * sum over clusters of |c|^2 (a device reduction over the cluster sizes).  It is the improved (cluster) estimator of the
+ * magnetisation's second moment: q <sum_s n_s^2> - N^2 = (q - 1) <sum_c |c|^2>, the quantity behind the moment-ratio
+ * check of PAPER.md:90.  n_clusters / largest_cluster may be NULL.  SW_ERR_STATE if no sweep since sw_init.          */
+int sw_measure_clusters(sw_ctx *ctx, uint64_t *n_clusters, uint64_t *largest_cluster, uint64_t sum_sq[2]);
+
 /* n x (one sweep, one measurement) without a host round trip per sweep; row k of `out`
  * (host uint64[n][3+q]) = energy_bonds, n_clusters, largest_cluster, mag_counts[0..q-1]
  * after sweep k.  Synchronises once at the end.                                                  */

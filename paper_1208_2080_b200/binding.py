@@ -26,7 +26,7 @@ _lib = None
 # every symbol include/sw.h declares (tests check that the library exports them all)
 SYMBOLS = [
     "sw_create", "sw_create_ex", "sw_workspace_bytes", "sw_create_ws", "sw_destroy", "sw_init",
-    "sw_set_state", "sw_sweep", "sw_measure", "sw_sweep_measure", "sw_sweep_measure_ex", "sw_get_spins", "sw_get_labels",
+    "sw_set_state", "sw_sweep", "sw_measure", "sw_measure_clusters", "sw_sweep_measure", "sw_sweep_measure_ex", "sw_get_spins", "sw_get_labels",
     "sw_get_bonds", "sw_get_rows", "sw_get_threshold", "sw_get_time", "sw_synchronize",
     "sw_get_stats", "sw_profile_begin", "sw_profile_end", "sw_profile_series", "sw_kernel_name", "sw_last_error",
     "sw_version",
@@ -81,6 +81,7 @@ def lib():
     l.sw_set_state.argtypes = [vp, vp, C.c_uint64]
     l.sw_sweep.argtypes = [vp, C.c_uint64]
     l.sw_measure.argtypes = [vp, u64p, u64p, u64p, u64p]
+    l.sw_measure_clusters.argtypes = [vp, u64p, u64p, u64p]
     l.sw_sweep_measure.argtypes = [vp, C.c_uint64, vp]
     l.sw_sweep_measure_ex.argtypes = [vp, C.c_uint64, vp, C.c_uint32]
     l.sw_get_spins.argtypes = [vp, vp]
@@ -195,6 +196,13 @@ class SwendsenWang:
         if clusters: out["n_clusters"] = int(nc.value)
         if largest: out["largest_cluster"] = int(big.value)
         return out
+
+    def measure_clusters(self):
+        """n_clusters, largest_cluster and sum over clusters of |c|^2 (a Python int: up to 2^64) of the last sweep."""
+        nc, big = C.c_uint64(), C.c_uint64()
+        sq = (C.c_uint64 * 2)()
+        self._chk(lib().sw_measure_clusters(self._h, C.byref(nc), C.byref(big), sq), "sw_measure_clusters")
+        return {"n_clusters": int(nc.value), "largest_cluster": int(big.value), "sum_sq": int(sq[0]) + (int(sq[1]) << 64)}
 
     def sweep_measure(self, n, what=OBS_ALL):
         """n x (sweep, measure); columns: energy_bonds, n_clusters, largest_cluster, mag_counts[q]."""

@@ -56,7 +56,7 @@ Plan make_plan(uint32_t L, uint32_t q, uint32_t flags)
     p.edges = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileEdges) : 0));
     p.tile_clusters = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * (sw::kFlipThreads / 32) * 4 : 0));
     p.draws = off;  off = align_up(off + (tiled_ok(L, flags) ? (N / 32) * sizeof(uint2) : 0));   // one uint2 per 8 x 4 block
-    p.row = off;    off = align_up(off + (3 + (size_t)q) * 8);
+    p.row = off;    off = align_up(off + (3 + (size_t)q + 2) * 8);   // + the two words of sum |c|^2 (sw_measure_clusters)
     p.flag = off;   off = align_up(off + 4);
     // scratch the read-back / measurement calls need, owned by the context (no cudaMalloc behind the caller's back):
     // a ring of observable rows for sw_sweep_measure, a staging buffer for sw_get_bonds, the pass counters of sw_get_stats
@@ -339,7 +339,7 @@ int ensure_flat(sw_ctx *c)
 }
 
 // Enqueue the observable kernels for the current state into the device row `row` (zeroed here).
-int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m, bool want_nc, bool want_big)
+int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m, bool want_nc, bool want_big, unsigned long long *c2 = nullptr)
 {
     const Params P = make_params(c, c->t);
     SW_CUDA(c, cudaMemsetAsync(row, 0, (3 + (size_t)c->q) * 8, c->stream));
@@ -370,7 +370,10 @@ int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m
         SW_CUDA(c, cudaMemsetAsync(c->d_sizes, 0, c->N * 4, c->stream));
         c->launches += 2;
         sw::k_cluster_sizes<<<grid_for(c, (c->N + 15) / 16, 256), 256, 0, c->stream>>>(c->d_labels, c->d_sizes, P);
-        sw::k_max_size<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_sizes, P, row);
+        if (c2) {
+            SW_CUDA(c, cudaMemsetAsync(c2, 0, 16, c->stream));
+            sw::k_size_moments<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_sizes, P, row, c2);
+        } else sw::k_max_size<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_sizes, P, row);
     }
     SW_CUDA(c, cudaGetLastError());
     return SW_OK;
@@ -553,6 +556,25 @@ int sw_measure(sw_ctx *c, uint64_t *energy_bonds, uint64_t *mag_counts, uint64_t
     if (n_clusters) *n_clusters = c->have_labels ? row[1] : 0;
     if (largest_cluster) *largest_cluster = c->have_labels ? row[2] : 0;
     if (mag_counts) for (uint32_t s = 0; s < c->q; ++s) mag_counts[s] = row[3 + s];
+    return SW_OK;
+}
+
+int sw_measure_clusters(sw_ctx *c, uint64_t *n_clusters, uint64_t *largest_cluster, uint64_t sum_sq[2])
+{
+    if (!c || !sum_sq) return SW_ERR_INVALID_ARG;
+    if (!c->have_labels) return fail(c, SW_ERR_STATE, "sw_measure_clusters: no sweep since sw_init");
+    DeviceGuard dg(c);
+    unsigned long long *c2 = c->d_row + 3 + c->q;
+    const int rc = enqueue_observe(c, c->d_row, false, false, true, true, c2);
+    if (rc != SW_OK) return rc;
+    std::vector<uint64_t> row(3 + c->q + 2);
+    SW_CUDA(c, cudaMemcpyAsync(row.data(), c->d_row, row.size() * 8, cudaMemcpyDeviceToHost, c->stream));
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    fix_row(c, row.data());
+    if (n_clusters) *n_clusters = row[1];
+    if (largest_cluster) *largest_cluster = row[2];
+    sum_sq[0] = row[3 + c->q]; sum_sq[1] = row[3 + c->q + 1];
+    if (row[1] == 1 && c->N == (1ull << 32)) { sum_sq[0] = 0; sum_sq[1] = 1; }   // one cluster of 2^32 sites: its uint32 counter wrapped
     return SW_OK;
 }
 

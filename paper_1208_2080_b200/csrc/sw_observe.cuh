@@ -188,4 +188,37 @@ __global__ void k_max_size(const uint32_t *__restrict__ sizes, Params P, unsigne
     if ((threadIdx.x & 31) == 0 && m) atomicMax(row + 2, (unsigned long long)m);
 }
 
+// Moments of the cluster-size distribution from sizes[] (only roots hold a count): row[2] = max, and the 128-bit sum of
+// squares c2[0] + 2^64 c2[1] = sum over clusters of |c|^2 -- the improved estimator of the susceptibility (the cluster
+// representation of <m^2>).  |c|^2 can reach 2^64 (one cluster of 2^32 sites), hence two words.
+__global__ void k_size_moments(const uint32_t *__restrict__ sizes, Params P, unsigned long long *row, unsigned long long *c2)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    uint32_t m = 0;
+    unsigned long long lo = 0, hi = 0;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < P.N; i += stride) {
+        const uint32_t sz = sizes[i];
+        if (!sz) continue;
+        m = max(m, sz);
+        const unsigned long long sq = (unsigned long long)sz * sz, before = lo;
+        lo += sq;
+        hi += lo < before;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        m = max(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
+        const unsigned long long olo = __shfl_xor_sync(0xFFFFFFFFu, lo, o), ohi = __shfl_xor_sync(0xFFFFFFFFu, hi, o), before = lo;
+        lo += olo;
+        hi += ohi + (lo < before);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (m) atomicMax(row + 2, (unsigned long long)m);
+        if (lo | hi) {
+            const unsigned long long old = atomicAdd(c2, lo);
+            if (old + lo < old) hi += 1;
+            if (hi) atomicAdd(c2 + 1, hi);
+        }
+    }
+}
+
 }  // namespace sw

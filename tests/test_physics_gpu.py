@@ -4,6 +4,7 @@ magnetization".  At the critical coupling of the 2D Ising model on a periodic sq
 <m^2>^2 / <m^4> tends to the universal value 0.856216 (Kamieniarz and Bloete, J. Phys. A 26 (1993) 201), i.e.
 <m^4> / <m^2>^2 = 1.16792; away from K_c it moves to 1 (ordered) or 3 (disordered)."""
 import math
+import os
 
 import numpy as np
 import pytest
@@ -46,3 +47,100 @@ def test_moment_ratio_orders_with_temperature():
     r_crit, _ = moment_ratio(64, kc, sweeps=4000, warm=300, seed=5)
     r_cold, _ = moment_ratio(64, 1.2 * kc, sweeps=4000, warm=300, seed=5)
     assert 2.5 < r_hot < 3.3 and 1.0 <= r_cold < 1.01 and r_cold < r_crit < r_hot
+
+
+# ---------------------------------------------------------------- the authors' own check, in full
+
+def moment_ratio_curve(L, Ks, sweeps, warm, seed):
+    """r(K) = <m^4> / <m^2>^2 with binned errors, one chain per coupling; plus the cluster (improved) estimator of <m^2>."""
+    out = []
+    for K in Ks:
+        g = SwendsenWang(L, 2, K, seed)
+        g.init("random")
+        g.sweep(warm)
+        rows = g.sweep_measure(sweeps)
+        g.close()
+        mag = rows[:, 3:5].astype(np.float64)
+        m = (mag[:, 0] - mag[:, 1]) / (L * L)
+        nb = 20
+        bins = np.array_split(m, nb)
+        r_bins = np.array([np.mean(b ** 4) / np.mean(b ** 2) ** 2 for b in bins])
+        out.append((np.mean(m ** 4) / np.mean(m ** 2) ** 2, np.std(r_bins, ddof=1) / math.sqrt(nb), np.mean(m ** 2)))
+    return np.array(out)
+
+
+def test_moment_ratio_curves_cross_at_the_critical_coupling():
+    """the authors "checked our code by plotting the temperature dependence of the moment ratio of
+    magnetization".  Curves of <m^4>/<m^2>^2 against K for L = 64, 128, 256, 512: below K_c the ratio grows with L (towards
+    3), above it falls (towards 1), and the curves of successive sizes cross at K_c = ln(1 + sqrt 2) within errors."""
+    kc = wl.k_critical(2)
+    rel = np.array([-0.03, -0.02, -0.01, -0.005, 0.0, 0.005, 0.01, 0.02, 0.03])
+    Ks = kc * (1.0 + rel)
+    sizes = [64, 128, 256, 512]
+    curves = {L: moment_ratio_curve(L, Ks, sweeps=12000 if L < 512 else 6000, warm=400, seed=7) for L in sizes}
+    lines = ["# <m^4>/<m^2>^2 of the 2D Ising model (q = 2 Potts) on the CUDA path, sw_sweep_measure every sweep; (K - K_c)/K_c per column",
+             "# L    " + "  ".join(f"{x:+.3f}         " for x in rel)]
+    for L in sizes:
+        lines.append(f"{L:<5d}  " + "  ".join(f"{r:.4f}+-{e:.4f}" for r, e, _ in curves[L]))
+    table = "\n".join(lines)
+    print(table)
+    out_dir = os.environ.get("SW_PHYSICS_TABLE_DIR")
+    if out_dir:
+        with open(os.path.join(out_dir, "moment_ratio_curves.txt"), "w") as f:
+            f.write(table + "\n")
+    i0 = int(np.flatnonzero(rel == 0.0)[0])
+    for L in sizes:                                            # at K_c: the universal value, for every size
+        r, e, _ = curves[L][i0]
+        assert abs(r - 1.0 / Q_UNIVERSAL) < max(5 * e, 0.02), (L, r, e)
+        assert np.all(np.diff(curves[L][:, 0]) < 3 * np.hypot(curves[L][1:, 1], curves[L][:-1, 1]))   # monotone in K within errors
+    for a, b in zip(sizes[:-1], sizes[1:]):
+        d = curves[b][:, 0] - curves[a][:, 0]
+        err = np.hypot(curves[b][:, 1], curves[a][:, 1])
+        lo, hi = rel < 0, rel > 0
+        # disordered side: the larger lattice has the larger ratio (both saturate at 3 far from K_c, so the clear separation
+        # is asked for next to K_c); ordered side: the smaller one
+        assert np.all(d[lo] > -3 * err[lo]) and d[i0 - 1] > 3 * err[i0 - 1], (a, b, d)
+        assert np.all(d[hi] < 3 * err[hi]) and d[i0 + 1] < -3 * err[i0 + 1], (a, b, d)
+        # the crossing: zero of the difference, by linear interpolation between the last positive and the first negative point
+        k = int(np.flatnonzero(d < 0)[0])
+        assert k > 0
+        x = rel[k - 1] + (rel[k] - rel[k - 1]) * d[k - 1] / (d[k - 1] - d[k])
+        assert abs(x) < 0.006, (a, b, x)                         # within 0.6 % of K_c (finite-size drift + statistical error)
+
+
+def test_sum_of_squared_cluster_sizes_and_the_improved_estimator():
+    # the device reduction against a plain bincount of the ORACLE's labels, and the identity that ties clusters to spins:
+    # q <sum_s n_s^2> - N^2 = (q - 1) <sum_c |c|^2>  (SURVEY.md sec. 8(c-7))
+    from oracle.binding import Oracle
+    for L, q in ((192, 2), (320, 3)):                           # cluster path and three-kernel path
+        K = wl.k_critical(q)
+        gpu, cpu = SwendsenWang(L, q, K, 5), Oracle(L, q, K, 5)
+        gpu.init("random"); cpu.init("random")
+        for _ in range(4):
+            gpu.sweep(1); cpu.sweep(1)
+            sizes = np.bincount(cpu.get_labels()).astype(object)
+            want = int(np.sum(sizes * sizes))
+            got = gpu.measure_clusters()
+            assert got["sum_sq"] == want and got["largest_cluster"] == int(max(sizes)) and got["n_clusters"] == int(np.count_nonzero(sizes))
+    # one cluster of all sites: |c|^2 = N^2
+    L = 256
+    g = SwendsenWang(L, 2, math.inf, 1)
+    g.init("ordered"); g.sweep(1)
+    assert g.measure_clusters() == {"n_clusters": 1, "largest_cluster": L * L, "sum_sq": (L * L) ** 2}
+    # the identity, in expectation, at criticality (L = 128, 6000 sweeps)
+    L, q = 128, 2
+    g = SwendsenWang(L, q, wl.k_critical(q), 9)
+    g.init("random"); g.sweep(300)
+    lhs, rhs = [], []
+    for _ in range(6000):
+        g.sweep(1)
+        rhs.append(g.measure_clusters()["sum_sq"])
+        n = g.measure(energy=False, clusters=False, largest=False)["mag_counts"]
+        lhs.append(q * sum(v * v for v in n) - (L * L) ** 2)
+    lhs, rhs = np.array(lhs, dtype=np.float64), (q - 1) * np.array(rhs, dtype=np.float64)
+    d = lhs - rhs
+    nb = 20
+    se = np.std([b.mean() for b in np.array_split(d, nb)], ddof=1) / math.sqrt(nb)
+    assert abs(d.mean()) < 5 * se and se < 0.05 * rhs.mean(), (d.mean(), se, rhs.mean())
+    # ... and the cluster estimator is the less noisy one (that is its point)
+    assert np.std(rhs) < np.std(lhs)
