@@ -241,6 +241,31 @@ int  sw_super_ipc_import(sw_super *s, uint32_t piece, const void *handle /* host
 int  sw_super_phase(sw_super *s, int phase /* 0, 1, 2; phase 2 advances the sweep counter */);
 int  sw_super_measure_phase(sw_super *s, int phase, uint32_t what /* SW_OBS_* */, uint64_t *part /* host [3+q], phase 2 */);
 
+/* --- the extension the paper names: embedded-cluster sweeps of the 2D classical XY model -----------------
+ * H = -J sum_<ij> s_i . s_j with unit vectors s_i; one sweep = the three steps of PAPER.md:40 on the Ising variables
+ * embedded by a random direction r (Wolff): a_i = s_i . r; bond <ij> active iff a_i a_j > 0 and
+ * draw < floor((1 - exp(-2 K a_i a_j)) 2^32); clusters labeled by their smallest site; a cluster is
+ * reflected, s -> s - 2 (s . r) r, iff floor(FLIP draw of its root * 2 / 2^32) == 1.  Draws: the Potts layout (BOND,
+ * FLIP, INIT) plus purpose 3 REFLECT (idx 0, sweep t, word 0): the angle of r is 2 pi (w0 + 1/2) / 2^32.
+ * Spins are double[L*L][2] (x, y); all arithmetic is IEEE double with explicit roundings (X1-X6), any L >= 2.
+ * sw_xy_init: ORDERED = all spins (1, 0); RANDOM = a point of (-1, 1)^2 from two INIT words (the other two if it lies
+ * outside the unit disc), normalised.  energy_sum = sum over bonds of s_i . s_j (E = -J energy_sum); mag = sum of spins;
+ * cluster statistics describe the bonds of the last sweep.  Device memory is owned by the library; all calls return a
+ * status; sw_xy_sweep is asynchronous on the context's stream, the read-backs synchronise.                              */
+typedef struct sw_xy sw_xy;
+int  sw_xy_create(sw_xy **out, uint32_t L, double K, uint64_t seed);
+void sw_xy_destroy(sw_xy *c);
+int  sw_xy_init(sw_xy *c, int mode);
+int  sw_xy_set_state(sw_xy *c, const double *spins /* host [L*L][2], finite */, uint64_t t);
+int  sw_xy_sweep(sw_xy *c, uint64_t n);
+int  sw_xy_measure(sw_xy *c, double *energy_sum, double mag[2], uint64_t *n_clusters, uint64_t *largest_cluster);
+int  sw_xy_get_spins(sw_xy *c, double *dst /* host [L*L][2] */);
+int  sw_xy_get_labels(sw_xy *c, uint32_t *dst /* host [L*L] */);
+int  sw_xy_get_bonds(sw_xy *c, uint8_t *dst /* host [L*L], bit0 right, bit1 down */);
+int  sw_xy_get_reflection(sw_xy *c, double r[2]);  /* the direction r of the last sweep */
+int  sw_xy_get_time(sw_xy *c, uint64_t *t);
+const char *sw_xy_last_error(const sw_xy *c);
+
 #ifdef __cplusplus
 }
 #endif

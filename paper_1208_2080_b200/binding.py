@@ -34,6 +34,8 @@ SYMBOLS = [
     "sw_super_get_spins", "sw_super_get_labels", "sw_super_get_bonds", "sw_super_get_time", "sw_super_synchronize",
     "sw_super_get_stats", "sw_super_last_error",
     "sw_create_super_rank", "sw_super_ipc_export", "sw_super_ipc_import", "sw_super_phase", "sw_super_measure_phase",
+    "sw_xy_create", "sw_xy_destroy", "sw_xy_init", "sw_xy_set_state", "sw_xy_sweep", "sw_xy_measure", "sw_xy_get_spins",
+    "sw_xy_get_labels", "sw_xy_get_bonds", "sw_xy_get_reflection", "sw_xy_get_time", "sw_xy_last_error",
 ]
 
 
@@ -111,6 +113,19 @@ def lib():
     l.sw_super_synchronize.argtypes = [vp]
     l.sw_super_get_stats.argtypes = [vp, C.POINTER(SuperStats)]
     l.sw_super_last_error.argtypes = [vp]; l.sw_super_last_error.restype = C.c_char_p
+    dp = C.POINTER(C.c_double)
+    l.sw_xy_create.argtypes = [C.POINTER(vp), C.c_uint32, C.c_double, C.c_uint64]
+    l.sw_xy_destroy.argtypes = [vp]; l.sw_xy_destroy.restype = None
+    l.sw_xy_init.argtypes = [vp, C.c_int]
+    l.sw_xy_set_state.argtypes = [vp, vp, C.c_uint64]
+    l.sw_xy_sweep.argtypes = [vp, C.c_uint64]
+    l.sw_xy_measure.argtypes = [vp, dp, dp, u64p, u64p]
+    l.sw_xy_get_spins.argtypes = [vp, vp]
+    l.sw_xy_get_labels.argtypes = [vp, vp]
+    l.sw_xy_get_bonds.argtypes = [vp, vp]
+    l.sw_xy_get_reflection.argtypes = [vp, dp]
+    l.sw_xy_get_time.argtypes = [vp, u64p]
+    l.sw_xy_last_error.argtypes = [vp]; l.sw_xy_last_error.restype = C.c_char_p
     for name in SYMBOLS:
         getattr(l, name)                         # AttributeError here = the library is stale
     _lib = l
@@ -367,3 +382,75 @@ class SuperLattice:
         s = SuperStats()
         self._chk(lib().sw_super_get_stats(self._h, C.byref(s)), "sw_super_get_stats")
         return {f: int(getattr(s, f)) for f, _ in SuperStats._fields_}
+
+
+class XYModel:
+    """Embedded-cluster sweeps of the 2D classical XY model; method names follow include/sw.h (`sw_xy_`)."""
+
+    def __init__(self, L, K, seed):
+        self.L, self.K, self.seed = int(L), float(K), int(seed)
+        self.N = self.L * self.L
+        self._h = C.c_void_p()
+        rc = lib().sw_xy_create(C.byref(self._h), self.L, self.K, self.seed)
+        if rc != OK:
+            self._h = C.c_void_p()
+            raise SwError(rc, "sw_xy_create")
+
+    def close(self):
+        if self._h:
+            lib().sw_xy_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _chk(self, rc, what):
+        if rc != OK:
+            msg = lib().sw_xy_last_error(self._h)
+            raise SwError(rc, what, msg.decode() if msg else "")
+
+    def init(self, mode):
+        self._chk(lib().sw_xy_init(self._h, {"ordered": INIT_ORDERED, "random": INIT_RANDOM}.get(mode, mode)), "sw_xy_init")
+
+    def set_state(self, spins, t):
+        s = np.ascontiguousarray(spins, dtype=np.float64).reshape(-1)
+        if s.size != 2 * self.N:
+            raise SwError(ERR_INVALID_ARG, "sw_xy_set_state", "wrong number of spin components")
+        self._chk(lib().sw_xy_set_state(self._h, s.ctypes.data, int(t)), "sw_xy_set_state")
+
+    def sweep(self, n=1):
+        self._chk(lib().sw_xy_sweep(self._h, int(n)), "sw_xy_sweep")
+
+    def measure(self):
+        e, nc, big = C.c_double(), C.c_uint64(), C.c_uint64()
+        m = (C.c_double * 2)()
+        self._chk(lib().sw_xy_measure(self._h, C.byref(e), m, C.byref(nc), C.byref(big)), "sw_xy_measure")
+        return {"energy_sum": float(e.value), "mag": [float(m[0]), float(m[1])], "n_clusters": int(nc.value), "largest_cluster": int(big.value)}
+
+    def get_spins(self):
+        out = np.empty((self.N, 2), dtype=np.float64)
+        self._chk(lib().sw_xy_get_spins(self._h, out.ctypes.data), "sw_xy_get_spins")
+        return out
+
+    def get_labels(self):
+        out = np.empty(self.N, dtype=np.uint32)
+        self._chk(lib().sw_xy_get_labels(self._h, out.ctypes.data), "sw_xy_get_labels")
+        return out
+
+    def get_bonds(self):
+        out = np.empty(self.N, dtype=np.uint8)
+        self._chk(lib().sw_xy_get_bonds(self._h, out.ctypes.data), "sw_xy_get_bonds")
+        return out
+
+    def get_reflection(self):
+        r = (C.c_double * 2)()
+        self._chk(lib().sw_xy_get_reflection(self._h, r), "sw_xy_get_reflection")
+        return float(r[0]), float(r[1])
+
+    def get_time(self):
+        t = C.c_uint64()
+        self._chk(lib().sw_xy_get_time(self._h, C.byref(t)), "sw_xy_get_time")
+        return int(t.value)

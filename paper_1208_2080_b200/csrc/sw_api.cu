@@ -754,3 +754,6 @@ const char *sw_last_error(const sw_ctx *c) { return c ? c->err.c_str() : "null c
 
 // the super-lattice decomposition: same translation unit, its own context type
 #include "sw_super.cuh"
+
+// the embedded-cluster XY extension
+#include "sw_xy.cuh"
