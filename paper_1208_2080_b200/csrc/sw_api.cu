@@ -13,6 +13,7 @@
 #include <string>
 #include <vector>
 
+#include "sw_host.h"
 #include "sw_common.cuh"
 #include "sw_generic.cuh"
 #include "sw_observe.cuh"
@@ -156,21 +157,7 @@ bool host_threshold(double K, uint64_t *T)
 
 Params make_params(const sw_ctx *c, uint64_t t)
 {
-    Params P{};
-    uint32_t k0 = (uint32_t)c->seed, k1 = (uint32_t)(c->seed >> 32);
-    for (int r = 0; r < 10; ++r) {
-        P.rk0[r] = k0; P.rk1[r] = k1;
-        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
-    }
-    P.L = c->L; P.q = c->q; P.t = (uint32_t)t; P.N = c->N;
-    P.thr_any = c->T ? 0xFFFFFFFFu : 0u;
-    P.thr_m1 = c->T ? (uint32_t)(c->T - 1) : 0u;
-    P.log2L = 0xFFFFFFFFu;
-    for (uint32_t b = 0; b < 17; ++b) if ((1u << b) == c->L) P.log2L = b;
-    P.divL_magic = ((1ull << 40) + c->L - 1) / c->L;
-    sw::sweep_keys(P, P.t, P.pk_t);
-    sw::sweep_keys(P, P.t + 1u, P.pk_n);
-    return P;
+    return swh::make_params(c->L, c->q, c->N, c->seed, c->T, t);
 }
 
 int grid_for(const sw_ctx *c, uint64_t items, int threads)
