@@ -344,21 +344,39 @@ def run_gpu(args):
     torch.cuda.synchronize()
     value_meas = N * m_steps / (e0.elapsed_time(e1) * 1e-3) / 1e9
 
-    # ---- end to end through the C ABI with HOST buffers: H2D of the spins, one sweep, D2H of the new spins
+    # ---- end to end through the C ABI with HOST buffers: H2D of the state, one sweep, D2H of the new state, every step.
+    # The state crosses PCIe in the library's packed form (sw_set_state_packed / sw_get_spins_packed: 1 bit per spin at
+    # q = 2), which is lossless and what a checkpoint would move; the byte-per-spin form is timed beside it.
+    bits = next(b for b in (1, 2, 4, 8) if q <= (1 << b))
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
-    host = torch.empty(N, dtype=torch.uint8, pin_memory=True)
-    sim.get_spins_ptr(host.data_ptr())
+    host = torch.empty(N * bits // 8, dtype=torch.uint8, pin_memory=True)
+    sim.get_spins_packed(bits, out=host.data_ptr())
     t_now = sim.get_time()
+    sim.set_state_packed(host.data_ptr(), bits, t_now)     # (untimed: one round trip so that every buffer has been touched)
     barrier()
     w0 = time.perf_counter()
     for k in range(e2e_steps):
-        sim.set_state_ptr(host.data_ptr(), t_now + k)      # H2D (+ on-device validation of the spin values)
+        sim.set_state_packed(host.data_ptr(), bits, t_now + k)     # H2D + unpack + validation of every value
         sim.sweep(1)
-        sim.get_spins_ptr(host.data_ptr())                 # D2H; synchronises
+        sim.get_spins_packed(bits, out=host.data_ptr())            # pack + D2H; synchronises
     barrier()
     e2e_s = time.perf_counter() - w0
     e2e_value = replicas.aggregate_throughput(N * e2e_steps, e2e_s, device="cuda")[2] / 1e9
     del host
+    e2e_unpacked = None
+    if world == 1:
+        host = torch.empty(N, dtype=torch.uint8, pin_memory=True)
+        sim.get_spins_ptr(host.data_ptr())
+        t_now = sim.get_time()
+        torch.cuda.synchronize()
+        w0 = time.perf_counter()
+        for k in range(min(2, e2e_steps)):
+            sim.set_state_ptr(host.data_ptr(), t_now + k)
+            sim.sweep(1)
+            sim.get_spins_ptr(host.data_ptr())
+        e2e_unpacked = {"value": N * min(2, e2e_steps) / (time.perf_counter() - w0) / 1e9, "unit": UNIT, "h2d_bytes_per_step": N, "d2h_bytes_per_step": N,
+                        "what": "sw_set_state + sw_sweep(1) + sw_get_spins, one byte per spin: PCIe-bound (8 GiB per step at L = 65536)"}
+        del host
 
     stats = sim.stats()
     if rank != 0:
@@ -450,8 +468,10 @@ def run_gpu(args):
                    "l2": f"working set {stats['device_bytes'] / 2**30:.1f} GiB >> 126 MB L2, no flush needed" if stats["device_bytes"] > (1 << 30)
                          else "working set fits L2: HBM roofline fractions are not meaningful at this size"},
         "clocks": clocks,
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N, "d2h_bytes_per_step": N, "steps": e2e_steps,
-                "what": "sw_set_state(host spins) + sw_sweep(1) + sw_get_spins(host) per step, pinned host memory"},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N * bits // 8, "d2h_bytes_per_step": N * bits // 8, "steps": e2e_steps,
+                "what": f"sw_set_state_packed(host, {bits} bit(s) per spin) + sw_sweep(1) + sw_get_spins_packed(host) per step, pinned host memory; "
+                        "input of step k + 1 = output of step k"},
+        "e2e_unpacked": e2e_unpacked,
         "gpu_launches": launches,
         "roofline": roofline,
         "roofline_alu": roofline_alu,

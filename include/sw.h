@@ -102,6 +102,13 @@ int sw_init(sw_ctx *ctx, int mode);
  * SW_ERR_INVALID_ARG (checked on the device); t <= 2^32 - 1.                                     */
 int sw_set_state(sw_ctx *ctx, const uint8_t *src, uint64_t t);
 
+/* The same state in packed form: `bits` in {1, 2, 4, 8} bits per spin with q <= 2^bits; site i occupies bits
+ * [bits (i % per), bits (i % per + 1)) of byte i / per, per = 8 / bits (little-endian inside the byte); L*L must be a
+ * multiple of 16.  A q = 2 lattice of 2^32 sites is 512 MiB instead of 4 GiB: the form to move a checkpoint over PCIe.
+ * src / dst: host, L*L*bits/8 bytes.  sw_set_state_packed validates every value (< q) like sw_set_state.            */
+int sw_set_state_packed(sw_ctx *ctx, const void *src, uint32_t bits, uint64_t t);
+int sw_get_spins_packed(sw_ctx *ctx, void *dst, uint32_t bits);
+
 /* --- the hot path -----------------------------------------------------------------------------
  * sw_sweep: n full sweeps (PAPER.md:40 steps 1-3), asynchronous on the context stream.
  * SW_ERR_STATE before sw_init/sw_set_state, or if t + n would pass 2^32 (the sweep field of the

@@ -26,7 +26,7 @@ _lib = None
 # every symbol include/sw.h declares (tests check that the library exports them all)
 SYMBOLS = [
     "sw_create", "sw_create_ex", "sw_workspace_bytes", "sw_create_ws", "sw_destroy", "sw_init",
-    "sw_set_state", "sw_sweep", "sw_measure", "sw_measure_clusters", "sw_sweep_measure", "sw_sweep_measure_ex", "sw_get_spins", "sw_get_labels",
+    "sw_set_state", "sw_set_state_packed", "sw_get_spins_packed", "sw_sweep", "sw_measure", "sw_measure_clusters", "sw_sweep_measure", "sw_sweep_measure_ex", "sw_get_spins", "sw_get_labels",
     "sw_get_bonds", "sw_get_rows", "sw_get_threshold", "sw_get_time", "sw_synchronize",
     "sw_get_stats", "sw_profile_begin", "sw_profile_end", "sw_profile_series", "sw_kernel_name", "sw_last_error",
     "sw_version",
@@ -81,6 +81,8 @@ def lib():
     l.sw_destroy.argtypes = [vp]; l.sw_destroy.restype = None
     l.sw_init.argtypes = [vp, C.c_int]
     l.sw_set_state.argtypes = [vp, vp, C.c_uint64]
+    l.sw_set_state_packed.argtypes = [vp, vp, C.c_uint32, C.c_uint64]
+    l.sw_get_spins_packed.argtypes = [vp, vp, C.c_uint32]
     l.sw_sweep.argtypes = [vp, C.c_uint64]
     l.sw_measure.argtypes = [vp, u64p, u64p, u64p, u64p]
     l.sw_measure_clusters.argtypes = [vp, u64p, u64p, u64p]
@@ -195,6 +197,26 @@ class SwendsenWang:
     def set_state_ptr(self, host_ptr, t):
         """As set_state, from a raw host pointer (e.g. a pinned torch tensor's data_ptr())."""
         self._chk(lib().sw_set_state(self._h, C.c_void_p(host_ptr), int(t)), "sw_set_state")
+
+    def set_state_packed(self, packed, bits, t):
+        """packed: uint8 array of L*L*bits/8 bytes, or a raw host pointer (int)."""
+        if isinstance(packed, int):
+            ptr = C.c_void_p(packed)
+        else:
+            a = np.ascontiguousarray(packed, dtype=np.uint8).reshape(-1)
+            if a.size != self.N * int(bits) // 8:
+                raise SwError(ERR_INVALID_ARG, "sw_set_state_packed", "wrong number of bytes")
+            ptr = C.c_void_p(a.ctypes.data)
+        self._chk(lib().sw_set_state_packed(self._h, ptr, int(bits), int(t)), "sw_set_state_packed")
+
+    def get_spins_packed(self, bits, out=None):
+        """Returns a uint8 array of L*L*bits/8 bytes; `out` may be a raw host pointer (int) instead."""
+        if isinstance(out, int):
+            self._chk(lib().sw_get_spins_packed(self._h, C.c_void_p(out), int(bits)), "sw_get_spins_packed")
+            return None
+        out = np.empty(self.N * int(bits) // 8, dtype=np.uint8) if out is None else out
+        self._chk(lib().sw_get_spins_packed(self._h, out.ctypes.data, int(bits)), "sw_get_spins_packed")
+        return out
 
     # -- hot path
     def sweep(self, n=1):

@@ -63,7 +63,7 @@ Plan make_plan(uint32_t L, uint32_t q, uint32_t flags)
     // a ring of observable rows for sw_sweep_measure, a staging buffer for sw_get_bonds, the pass counters of sw_get_stats
     p.rows_cap = std::max<size_t>(16, std::min<size_t>(4096, (256u << 10) / ((3 + (size_t)q) * 8)));
     p.rows = off;   off = align_up(off + p.rows_cap * (3 + (size_t)q) * 8);
-    p.stage_bytes = (size_t)std::min<uint64_t>(N, 32ull << 20);
+    p.stage_bytes = (size_t)std::max<uint64_t>(512, (std::min<uint64_t>(N, 32ull << 20) + 511) / 512 * 512);   // two 256-byte-aligned halves
     p.stage = off;  off = align_up(off + p.stage_bytes);
     p.counters = off; off = align_up(off + sizeof(sw::PassCounters));
     // the 4N-byte cluster-size scratch of sw_measure(largest_cluster): part of the workspace only on request
@@ -500,6 +500,55 @@ int sw_set_state(sw_ctx *c, const uint8_t *src, uint64_t t)
     c->have_labels = false; c->labels_flat = false;
     if (bad) { c->have_spins = false; return fail(c, SW_ERR_INVALID_ARG, "sw_set_state: spin value >= q"); }
     c->t = t; c->have_spins = true;
+    return SW_OK;
+}
+
+static bool packed_ok(const sw_ctx *c, uint32_t bits)
+{
+    return (bits == 1 || bits == 2 || bits == 4 || bits == 8) && c->q <= (1u << bits) && c->N % 16 == 0;
+}
+
+int sw_set_state_packed(sw_ctx *c, const void *src, uint32_t bits, uint64_t t)
+{
+    if (!c || !src || t > 0xFFFFFFFFull) return fail(c, SW_ERR_INVALID_ARG, "sw_set_state_packed: bad argument");
+    if (!packed_ok(c, bits)) return fail(c, SW_ERR_INVALID_ARG, "sw_set_state_packed: bits must be 1, 2, 4 or 8 with q <= 2^bits, and L*L a multiple of 16");
+    DeviceGuard dg(c);
+    // the packed image is staged in the label array (the labels of the last sweep are forgotten by a new state anyway)
+    uint8_t *staged = reinterpret_cast<uint8_t *>(c->d_labels);
+    SW_CUDA(c, cudaMemcpyAsync(staged, src, (size_t)(c->N / 8 * bits), cudaMemcpyHostToDevice, c->stream));
+    SW_CUDA(c, cudaMemsetAsync(c->d_flag, 0, 4, c->stream));
+    const Params P = make_params(c, 0);
+    c->launches += 1;
+    sw::k_unpack_spins<<<grid_for(c, c->N / 16, 256), 256, 0, c->stream>>>(staged, c->d_spins, P, bits, c->d_flag);
+    uint32_t bad = 0;
+    SW_CUDA(c, cudaMemcpyAsync(&bad, c->d_flag, 4, cudaMemcpyDeviceToHost, c->stream));
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->have_labels = false; c->labels_flat = false;
+    if (bad) { c->have_spins = false; return fail(c, SW_ERR_INVALID_ARG, "sw_set_state_packed: spin value >= q"); }
+    c->t = t; c->have_spins = true;
+    return SW_OK;
+}
+
+int sw_get_spins_packed(sw_ctx *c, void *dst, uint32_t bits)
+{
+    if (!c || !dst) return fail(c, SW_ERR_INVALID_ARG, "sw_get_spins_packed: bad argument");
+    if (!packed_ok(c, bits)) return fail(c, SW_ERR_INVALID_ARG, "sw_get_spins_packed: bits must be 1, 2, 4 or 8 with q <= 2^bits, and L*L a multiple of 16");
+    if (!c->have_spins) return fail(c, SW_ERR_STATE, "no spins");
+    DeviceGuard dg(c);
+    // packed in chunks through the context's staging buffer, two halves in flight
+    const uint64_t n_groups = c->N / 16, bytes_per_group = 2ull * bits;
+    const uint64_t half = std::max<uint64_t>(1, (c->stage_bytes / 2) / bytes_per_group);      // groups per half
+    uint64_t done = 0;
+    for (int k = 0; done < n_groups; ++k) {
+        const uint64_t m = std::min(half, n_groups - done);
+        uint8_t *buf = c->d_stage + (k & 1) * (c->stage_bytes / 2);
+        c->launches += 1;
+        sw::k_pack_spins<<<grid_for(c, m, 256), 256, 0, c->stream>>>(c->d_spins, buf, done, m, bits);
+        SW_CUDA(c, cudaMemcpyAsync((uint8_t *)dst + done * bytes_per_group, buf, (size_t)(m * bytes_per_group), cudaMemcpyDeviceToHost, c->stream));
+        done += m;
+    }
+    SW_CUDA(c, cudaStreamSynchronize(c->stream));
+    SW_CUDA(c, cudaGetLastError());
     return SW_OK;
 }
 

@@ -32,6 +32,59 @@ __global__ void k_validate_spins(const uint8_t *__restrict__ spins, Params P, ui
     if (__any_sync(0xFFFFFFFFu, bad) && (threadIdx.x & 31) == 0) atomicOr(flag, 1u);
 }
 
+// --- packed spin states (sw_set_state_packed / sw_get_spins_packed): `bits` in {1, 2, 4, 8} per spin, site i in bits
+// [bits (i % per), bits (i % per + 1)) of byte i / per, per = 8 / bits.  One thread per 16 sites (a uint4 of spins).
+__global__ void k_unpack_spins(const uint8_t *__restrict__ packed, uint8_t *__restrict__ spins, Params P, uint32_t bits, uint32_t *flag)
+{
+    const uint64_t n_groups = P.N >> 4, stride = (uint64_t)gridDim.x * blockDim.x;   // N % 16 == 0 (checked by the caller)
+    const uint32_t mask = (1u << bits) - 1u;
+    bool bad = false;
+    for (uint64_t g = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; g < n_groups; g += stride) {
+        unsigned long long w = 0;                            // the 16 * bits <= 128 bits of this group; 8 bits per spin: two loads
+        uint32_t out[4];
+        if (bits == 8) {
+            const uint4 v = *reinterpret_cast<const uint4 *>(packed + (g << 4));
+            out[0] = v.x; out[1] = v.y; out[2] = v.z; out[3] = v.w;
+        } else {
+            if (bits == 1) w = *reinterpret_cast<const uint16_t *>(packed + (g << 1));
+            else if (bits == 2) w = *reinterpret_cast<const uint32_t *>(packed + (g << 2));
+            else w = *reinterpret_cast<const unsigned long long *>(packed + (g << 3));
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                uint32_t o = 0;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) o |= (uint32_t)((w >> (bits * (4 * k + j))) & mask) << (8 * j);
+                out[k] = o;
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) bad |= ((out[k] >> (8 * j)) & 0xFFu) >= P.q;
+        *reinterpret_cast<uint4 *>(spins + (g << 4)) = make_uint4(out[0], out[1], out[2], out[3]);
+    }
+    if (__any_sync(0xFFFFFFFFu, bad) && (threadIdx.x & 31) == 0) atomicOr(flag, 1u);
+}
+
+__global__ void k_pack_spins(const uint8_t *__restrict__ spins, uint8_t *__restrict__ packed, uint64_t first_group, uint64_t n_groups, uint32_t bits)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t k = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n_groups; k += stride) {
+        const uint64_t g = first_group + k;
+        const uint4 v = *reinterpret_cast<const uint4 *>(spins + (g << 4));
+        const uint32_t in[4] = {v.x, v.y, v.z, v.w};
+        if (bits == 8) { *reinterpret_cast<uint4 *>(packed + (k << 4)) = v; continue; }
+        unsigned long long w = 0;
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) w |= (unsigned long long)((in[a] >> (8 * j)) & 0xFFu) << (bits * (4 * a + j));
+        if (bits == 1) *reinterpret_cast<uint16_t *>(packed + (k << 1)) = (uint16_t)w;
+        else if (bits == 2) *reinterpret_cast<uint32_t *>(packed + (k << 2)) = (uint32_t)w;
+        else *reinterpret_cast<unsigned long long *>(packed + (k << 3)) = w;
+    }
+}
+
 // --- step (1): bonds, one thread per 16-site word -----------------------------------------------
 
 __global__ void k_bonds_generic(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds, Params P)

@@ -429,3 +429,50 @@ def test_sweep_measure_mask_and_series():
     ref = Oracle(64, 2, 0.5, 1)
     many.init("random"); ref.init("random")
     assert np.array_equal(many.sweep_measure(5000)[::97], ref.sweep_measure(5000)[::97])
+
+
+def pack_spins(spins, bits):
+    """Reference packing in numpy: site i in bits [bits (i % per), ...) of byte i // per."""
+    per = 8 // bits
+    s = np.asarray(spins, dtype=np.uint8).reshape(-1, per).astype(np.uint32)
+    out = np.zeros(s.shape[0], dtype=np.uint32)
+    for j in range(per):
+        out |= s[:, j] << (bits * j)
+    return out.astype(np.uint8)
+
+
+@pytest.mark.parametrize("L,q,bits", [(64, 2, 1), (192, 2, 2), (128, 3, 2), (128, 4, 2), (64, 10, 4), (96, 16, 4), (64, 200, 8), (320, 2, 1), (20, 2, 1)])
+def test_packed_state_transfer(L, q, bits):
+    K = wl.k_critical(q)
+    spins = wl.spins_uniform_random(L, q, 17)
+    a, b, cpu = SwendsenWang(L, q, K, 3), SwendsenWang(L, q, K, 3), Oracle(L, q, K, 3)
+    a.set_state(spins, 4); cpu.set_state(spins, 4)
+    b.set_state_packed(pack_spins(spins, bits), bits, 4)
+    assert np.array_equal(b.get_spins(), spins.reshape(-1))
+    a.sweep(2); b.sweep(2); cpu.sweep(2)
+    compare_after_sweep(b, cpu, f"(packed state, bits={bits})")
+    assert np.array_equal(b.get_spins_packed(bits), pack_spins(a.get_spins(), bits))
+    if bits < 8:
+        assert np.array_equal(b.get_spins_packed(8), a.get_spins())
+    # a packed image can hold values >= q when q is not a power of two: rejected like sw_set_state does
+    if q < (1 << bits):
+        bad = spins.copy().reshape(-1); bad[L * L // 2] = q
+        with pytest.raises(sw.SwError) as e:
+            b.set_state_packed(pack_spins(bad, bits), bits, 0)
+        assert e.value.code == sw.ERR_INVALID_ARG
+    if bits > 1 or q > 2:
+        with pytest.raises(sw.SwError):
+            b.get_spins_packed(1) if q > 2 else b.get_spins_packed(3)
+
+
+def test_packed_state_needs_enough_bits_and_a_multiple_of_16_sites():
+    g = SwendsenWang(64, 5, 1.0, 1)
+    g.init("random")
+    for bits in (1, 2, 3, 16):
+        with pytest.raises(sw.SwError) as e:
+            g.get_spins_packed(bits)
+        assert e.value.code == sw.ERR_INVALID_ARG
+    h = SwendsenWang(6, 2, 1.0, 1)                              # 36 sites: not a multiple of 16
+    h.init("random")
+    with pytest.raises(sw.SwError):
+        h.get_spins_packed(1)
