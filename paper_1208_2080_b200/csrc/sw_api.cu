@@ -105,6 +105,8 @@ struct sw_ctx {
     bool count_passes = false;
     uint32_t *d_sizes = nullptr;          // 4N-byte scratch for cluster sizes: in the workspace (SW_FLAG_WS_CLUSTER_SIZES) or
     bool owns_sizes = false;              // allocated once by the first sw_measure(largest_cluster)
+    bool sizes_zero = false;              // d_sizes is all zero (k_max_size_zero leaves it so; k_tile_flip_sizes relies on it)
+    uint64_t sizes_t = ~0ull;             // == t: d_sizes holds the cluster sizes of the last sweep, counted by k_tile_flip_sizes
     uint64_t launches = 0, sweeps = 0;
     int num_sms = 148;
     // profiling: events are created once and reused (no cudaEventCreate inside a timed region after the first pass)
@@ -200,6 +202,7 @@ int sweep_cluster(sw_ctx *c, uint64_t n, uint32_t what, unsigned long long *d_ro
         SW_CUDA(c, cudaMalloc(&c->d_sizes, c->N * 4));
         c->owns_sizes = true;
     }
+    if (what & SW_OBS_LARGEST) c->sizes_zero = false;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = tgrid; cfg.blockDim = dim3(sw::kClusterThreads); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
     cudaLaunchAttribute attr[1];
@@ -242,8 +245,25 @@ bool cluster_path_ok(sw_ctx *c)
     return true;
 }
 
-// count_clusters: the flip kernel also counts the canonical roots (wanted for the last sweep before a measurement)
-int sweep_once(sw_ctx *c, bool count_clusters)
+// the cluster-size counters: there, and all zero
+int ensure_sizes_zero(sw_ctx *c)
+{
+    if (!c->d_sizes) {                   // not part of the workspace (no SW_FLAG_WS_CLUSTER_SIZES): allocated once, kept until sw_destroy
+        SW_CUDA(c, cudaMalloc(&c->d_sizes, c->N * 4));
+        c->owns_sizes = true;
+        c->sizes_zero = false;
+    }
+    if (!c->sizes_zero) {
+        SW_CUDA(c, cudaMemsetAsync(c->d_sizes, 0, c->N * 4, c->stream));
+        c->sizes_zero = true;
+    }
+    return SW_OK;
+}
+
+// count_clusters: the flip kernel also counts the canonical roots (wanted for the last sweep before a measurement);
+// sizes_row != nullptr (a zeroed row of observables): it counts the cluster sizes as well (k_tile_flip_sizes) and raises
+// sizes_row[2] to the largest cluster that lies inside one tile; the rest is in d_sizes for k_max_size_zero
+int sweep_once(sw_ctx *c, bool count_clusters, unsigned long long *sizes_row = nullptr)
 {
     const Params P = make_params(c, c->t);
     if (c->tiled) {
@@ -258,6 +278,15 @@ int sweep_once(sw_ctx *c, bool count_clusters)
         { Timed tm(c, SLOT_MERGE);
           auto merge = c->count_passes ? sw::k_tile_merge<true> : sw::k_tile_merge<false>;
           merge<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_edges, P, tiles, c->d_counters); }
+        const bool with_sizes = sizes_row && !c->lazy && !c->count_passes;
+        if (with_sizes) {
+            const int rc = ensure_sizes_zero(c);
+            if (rc != SW_OK) return rc;
+            Timed tm(c, SLOT_FLIP);
+            sw::k_tile_flip_sizes<<<tgrid, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, c->d_draws, c->d_sizes, sizes_row);
+            c->sizes_zero = false;
+            c->sizes_t = c->t + 1;
+        } else
         { Timed tm(c, SLOT_FLIP);
           auto flip = c->count_passes ? (c->lazy ? sw::k_tile_flip<false, true, true, true> : sw::k_tile_flip<true, true, true, true>)
                     : c->lazy ? (count_clusters ? sw::k_tile_flip<false, true, true> : sw::k_tile_flip<false, true, false>)
@@ -326,10 +355,12 @@ int ensure_flat(sw_ctx *c)
 }
 
 // Enqueue the observable kernels for the current state into the device row `row` (zeroed here).
-int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m, bool want_nc, bool want_big, unsigned long long *c2 = nullptr)
+// row_is_zero: the caller zeroed the row already (and k_tile_flip_sizes may have put the largest tile-local cluster into row[2])
+int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m, bool want_nc, bool want_big, unsigned long long *c2 = nullptr,
+                    bool row_is_zero = false)
 {
     const Params P = make_params(c, c->t);
-    SW_CUDA(c, cudaMemsetAsync(row, 0, (3 + (size_t)c->q) * 8, c->stream));
+    if (!row_is_zero) SW_CUDA(c, cudaMemsetAsync(row, 0, (3 + (size_t)c->q) * 8, c->stream));
     const bool cl = c->have_labels;
     uint32_t want = (want_e ? 1u : 0u) | (want_m ? 2u : 0u) | ((cl && (want_nc || want_big)) ? 4u : 0u);
     if ((want & 4u) && c->tiled) {      // the flip kernel of the last sweep left one count per tile: no pass over labels[]
@@ -345,21 +376,29 @@ int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m
         else
             sw::k_observe_scalar<<<grid_for(c, c->N, sw::kObsThreads), sw::kObsThreads, 0, c->stream>>>(c->d_spins, c->d_labels, P, want, row);
     }
-    if (cl && want_big) {
+    if (cl && want_big && c->tiled && c->sizes_t == c->t && !c2) {
+        // the flip kernel of the last sweep counted the sizes: clusters inside one tile are in row[2] already, the others in d_sizes
+        c->launches += 1;
+        sw::k_max_size_zero<<<grid_for(c, c->N / 4, 256), 256, 0, c->stream>>>(c->d_sizes, P, row);
+        c->sizes_zero = true;
+        c->sizes_t = ~0ull;
+    } else if (cl && want_big) {
         if (c->tiled) {          // cluster sizes need root pointers: on the tiled path labels[] holds tile-local ids until flattened
             const int rc = ensure_flat(c);
             if (rc != SW_OK) return rc;
         }
-        if (!c->d_sizes) {               // not part of the workspace (no SW_FLAG_WS_CLUSTER_SIZES): allocated once, kept until sw_destroy
-            SW_CUDA(c, cudaMalloc(&c->d_sizes, c->N * 4));
-            c->owns_sizes = true;
-        }
-        SW_CUDA(c, cudaMemsetAsync(c->d_sizes, 0, c->N * 4, c->stream));
+        c->sizes_t = ~0ull;
+        const int rc = ensure_sizes_zero(c);
+        if (rc != SW_OK) return rc;
         c->launches += 2;
+        c->sizes_zero = false;
         sw::k_cluster_sizes<<<grid_for(c, (c->N + 15) / 16, 256), 256, 0, c->stream>>>(c->d_labels, c->d_sizes, P);
         if (c2) {
             SW_CUDA(c, cudaMemsetAsync(c2, 0, 16, c->stream));
             sw::k_size_moments<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_sizes, P, row, c2);
+        } else if (c->N % 4 == 0) {
+            sw::k_max_size_zero<<<grid_for(c, c->N / 4, 256), 256, 0, c->stream>>>(c->d_sizes, P, row);
+            c->sizes_zero = true;
         } else sw::k_max_size<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_sizes, P, row);
     }
     SW_CUDA(c, cudaGetLastError());
@@ -481,7 +520,7 @@ int sw_init(sw_ctx *c, int mode)
         sw::k_init_random<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_spins, P);
         SW_CUDA(c, cudaGetLastError());
     } else return fail(c, SW_ERR_INVALID_ARG, "sw_init: unknown mode");
-    c->t = 0; c->have_spins = true; c->have_labels = false; c->labels_flat = false;
+    c->t = 0; c->have_spins = true; c->have_labels = false; c->labels_flat = false; c->sizes_t = ~0ull;
     return SW_OK;
 }
 
@@ -497,7 +536,7 @@ int sw_set_state(sw_ctx *c, const uint8_t *src, uint64_t t)
     uint32_t bad = 0;
     SW_CUDA(c, cudaMemcpyAsync(&bad, c->d_flag, 4, cudaMemcpyDeviceToHost, c->stream));
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
-    c->have_labels = false; c->labels_flat = false;
+    c->have_labels = false; c->labels_flat = false; c->sizes_t = ~0ull;
     if (bad) { c->have_spins = false; return fail(c, SW_ERR_INVALID_ARG, "sw_set_state: spin value >= q"); }
     c->t = t; c->have_spins = true;
     return SW_OK;
@@ -523,7 +562,7 @@ int sw_set_state_packed(sw_ctx *c, const void *src, uint32_t bits, uint64_t t)
     uint32_t bad = 0;
     SW_CUDA(c, cudaMemcpyAsync(&bad, c->d_flag, 4, cudaMemcpyDeviceToHost, c->stream));
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
-    c->have_labels = false; c->labels_flat = false;
+    c->have_labels = false; c->labels_flat = false; c->sizes_t = ~0ull;
     if (bad) { c->have_spins = false; return fail(c, SW_ERR_INVALID_ARG, "sw_set_state_packed: spin value >= q"); }
     c->t = t; c->have_spins = true;
     return SW_OK;
@@ -630,10 +669,15 @@ int sw_sweep_measure_ex(sw_ctx *c, uint64_t n, uint64_t *out, uint32_t what)
     for (uint64_t done = 0; done < n && rc == SW_OK;) {
         const uint64_t m = (n - done < chunk_max) ? n - done : chunk_max;
         if (c->cluster) rc = sweep_cluster(c, m, what, d_rows);
-        else for (uint64_t k = 0; k < m && rc == SW_OK; ++k) {
-            rc = sweep_once(c, (what & (SW_OBS_CLUSTERS | SW_OBS_LARGEST)) != 0);
-            if (rc == SW_OK) rc = enqueue_observe(c, d_rows + k * stride, (what & SW_OBS_ENERGY) != 0, (what & SW_OBS_MAG) != 0,
-                                                  (what & (SW_OBS_CLUSTERS | SW_OBS_LARGEST)) != 0, (what & SW_OBS_LARGEST) != 0);
+        else {
+            cudaError_t e0 = cudaMemsetAsync(d_rows, 0, (size_t)m * stride * 8, c->stream);
+            if (e0 != cudaSuccess) rc = cuda_fail(c, e0, "sw_sweep_measure memset");
+            for (uint64_t k = 0; k < m && rc == SW_OK; ++k) {
+                unsigned long long *row = d_rows + k * stride;
+                rc = sweep_once(c, (what & (SW_OBS_CLUSTERS | SW_OBS_LARGEST)) != 0, (c->tiled && (what & SW_OBS_LARGEST)) ? row : nullptr);
+                if (rc == SW_OK) rc = enqueue_observe(c, row, (what & SW_OBS_ENERGY) != 0, (what & SW_OBS_MAG) != 0,
+                                                      (what & (SW_OBS_CLUSTERS | SW_OBS_LARGEST)) != 0, (what & SW_OBS_LARGEST) != 0, nullptr, true);
+            }
         }
         if (rc == SW_OK) {
             cudaError_t e = cudaMemcpyAsync(out + done * stride, d_rows, (size_t)m * stride * 8, cudaMemcpyDeviceToHost, c->stream);

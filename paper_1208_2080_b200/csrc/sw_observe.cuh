@@ -188,6 +188,24 @@ __global__ void k_max_size(const uint32_t *__restrict__ sizes, Params P, unsigne
     if ((threadIdx.x & 31) == 0 && m) atomicMax(row + 2, (unsigned long long)m);
 }
 
+// the same, and every counter that was read non-zero is set back to zero: sizes[] stays all zero between measurements
+// (k_tile_flip_sizes relies on that), without a memset of 4N bytes per measurement
+__global__ void k_max_size_zero(uint32_t *__restrict__ sizes, Params P, unsigned long long *row)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x * 4;
+    uint32_t m = 0;
+    for (uint64_t i = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4; i < P.N; i += stride) {    // N % 4 == 0 on the tiled path
+        const uint4 v = *reinterpret_cast<const uint4 *>(sizes + i);
+        if (v.x | v.y | v.z | v.w) {
+            m = max(m, max(max(v.x, v.y), max(v.z, v.w)));
+            *reinterpret_cast<uint4 *>(sizes + i) = make_uint4(0, 0, 0, 0);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(row + 2, (unsigned long long)m);
+}
+
 // Moments of the cluster-size distribution from sizes[] (only roots hold a count): row[2] = max, and the 128-bit sum of
 // squares c2[0] + 2^64 c2[1] = sum over clusters of |c|^2 -- the improved estimator of the susceptibility (the cluster
 // representation of <m^2>).  |c|^2 can reach 2^64 (one cluster of 2^32 sites), hence two words.

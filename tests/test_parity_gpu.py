@@ -476,3 +476,35 @@ def test_packed_state_needs_enough_bits_and_a_multiple_of_16_sites():
     h.init("random")
     with pytest.raises(sw.SwError):
         h.get_spins_packed(1)
+
+
+@pytest.mark.parametrize("L,q,K,start", [(320, 3, wl.k_critical(3), "random"), (448, 10, wl.k_critical(10) * 0.995, "random"),
+                                         (384, 2, wl.k_critical(2), "ordered"), (320, 2, math.inf, "ordered"), (320, 4, 0.0, "random"),
+                                         (192, 2, wl.k_critical(2), "random")])
+def test_series_with_cluster_sizes_counted_in_the_flip_kernel(L, q, K, start):
+    # sw_sweep_measure with the largest cluster on the three-kernel path: the sizes are counted by k_tile_flip_sizes
+    # (clusters inside one tile never touch global memory); every row must equal the oracle's, whatever is asked before and after
+    flags = sw.FLAG_NO_CLUSTER_PATH
+    gpu, cpu = SwendsenWang(L, q, K, 12, flags=flags), Oracle(L, q, K, 12)
+    gpu.init(start); cpu.init(start)
+    assert np.array_equal(gpu.sweep_measure(6), cpu.sweep_measure(6))
+    assert gpu.measure() == cpu.measure()                                        # the separate pass, right after
+    want = cpu.sweep_measure(4)
+    got = gpu.sweep_measure(4, sw.OBS_LARGEST)
+    assert np.array_equal(got[:, 1:3], want[:, 1:3])
+    gpu.sweep(2); cpu.sweep(2)
+    compare_after_sweep(gpu, cpu, "(after the series)")
+    assert np.array_equal(gpu.sweep_measure(3), cpu.sweep_measure(3))
+    assert gpu.measure_clusters()["largest_cluster"] == cpu.measure()["largest_cluster"]
+
+
+def test_cluster_sizes_in_the_flip_kernel_on_adversarial_lattices():
+    L = 320
+    for name, spins in wl.crafted_lattices(L, 3).items():
+        gpu, cpu = SwendsenWang(L, 3, math.inf, 1), Oracle(L, 3, math.inf, 1)
+        gpu.set_state(spins, 2); cpu.set_state(spins, 2)
+        assert np.array_equal(gpu.sweep_measure(2), cpu.sweep_measure(2)), name
+    big = SwendsenWang(1024, 2, wl.k_critical(2), 3, flags=sw.FLAG_WS_CLUSTER_SIZES)
+    ref = Oracle(1024, 2, wl.k_critical(2), 3)
+    big.init("ordered"); ref.init("ordered")
+    assert np.array_equal(big.sweep_measure(5, sw.OBS_CLUSTERS | sw.OBS_LARGEST)[:, 1:3], ref.sweep_measure(5)[:, 1:3])
