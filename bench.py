@@ -446,6 +446,31 @@ def run_gpu(args):
             except Exception as e:                                   # a failed side measurement must not lose the headline line
                 other[name] = {"error": repr(e)}
 
+    # ---- the super-lattice decomposition on ONE device: 2 x 2 pieces of the ncu-sized lattice, all on
+    # this GPU -- what the two-stage labeling (stage 2 over the boundary sites, resolve pass, event-ordered phases) costs next
+    # to the single-lattice path on the same sites.  The NVLink path itself cannot be measured on a one-GPU box.
+    if other is not None:
+        try:
+            from paper_1208_2080_b200.binding import SuperLattice
+            cs = wl.CONFIGS["p_L16384_q2"]
+            sup = SuperLattice(cs["L"], cs["q"], cs["K"], cs["seed"], 2, 2)
+            sup.init(cs["start"]); sup.sweep(30); sup.synchronize()
+            t0 = time.perf_counter(); sup.sweep(20); sup.synchronize(); dt = time.perf_counter() - t0
+            st = sup.stats()
+            sup.close()
+            one = SwendsenWang(cs["L"], cs["q"], cs["K"], cs["seed"])
+            one.init(cs["start"]); one.sweep(30); one.synchronize()
+            t0 = time.perf_counter(); one.sweep(20); one.synchronize(); dt1 = time.perf_counter() - t0
+            one.close()
+            other["super_2x2_L16384_q2_one_device"] = {
+                "flips_per_ns": cs["L"] ** 2 * 20 / dt / 1e9, "ms_per_sweep": dt / 20 * 1e3,
+                "single_lattice_flips_per_ns": cs["L"] ** 2 * 20 / dt1 / 1e9,
+                "inter_piece_links_per_sweep": st["inter_links"] / st["sweeps"], "inter_piece_label_loads_per_sweep": st["inter_hops"] / st["sweeps"],
+                "resolved_links_per_sweep": st["resolved_links"] / st["sweeps"], "boundary_sites_per_piece": st["boundary_sites_per_piece"],
+                "what": "wall clock around 20 sweeps + synchronize, all four pieces on this GPU; NVLink unmeasured"}
+        except Exception as e:
+            other["super_2x2_L16384_q2_one_device"] = {"error": repr(e)}
+
     # ---- the oracle on this box's host cores (reported baseline, rank 0, N = 1 only), on equilibrated lattices
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:

@@ -123,3 +123,15 @@ def test_non_power_of_two_size_and_state_machine():
     for bad in ((3, 3), (0, 1), (9, 9)):
         with pytest.raises(sw.SwError):
             SuperLattice(512, 2, 0.5, 1, *bad)
+
+
+def test_config4_size_q10_in_2x2_pieces_one_transition():
+    # BASELINE config 4 (L = 16384, q = 10, just below K_c) in 2 x 2 pieces of 8192^2: one equilibrated transition against the oracle
+    c = wl.CONFIGS["c4_L16384_q10_below"]
+    sup = SuperLattice(c["L"], c["q"], c["K"], c["seed"], 2, 2)
+    cpu = Oracle(c["L"], c["q"], c["K"], c["seed"])
+    sup.init(c["start"])
+    sup.sweep(40)
+    cpu.set_state(sup.get_spins(), sup.get_time())
+    sup.sweep(1); cpu.sweep(1)
+    compare(sup, cpu, "(c4 below, 2x2 pieces, t = 40)")
