@@ -91,7 +91,9 @@ int sw_create_ex(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed, 
 size_t sw_workspace_bytes(uint32_t L, uint32_t q, uint32_t flags);
 int sw_create_ws(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed, uint32_t flags,
                  void *dev_ws, size_t ws_bytes, void *cuda_stream);
-void sw_destroy(sw_ctx *ctx);                      /* NULL is allowed */
+/* Frees the context and the device memory the library allocated (a lent workspace stays the caller's); waits for the
+ * context's stream first.  NULL is allowed.  (BASELINE.json north_star lists sw_destroy among the seven calls.)     */
+void sw_destroy(sw_ctx *ctx);
 
 /* --- state ------------------------------------------------------------------------------------
  * sw_init: ORDERED = all spins 0; RANDOM = spin_i = floor(Philox(INIT, i).w0 * q / 2^32).
@@ -142,13 +144,16 @@ enum { SW_OBS_ENERGY = 1, SW_OBS_MAG = 2, SW_OBS_CLUSTERS = 4, SW_OBS_LARGEST = 
 int sw_sweep_measure_ex(sw_ctx *ctx, uint64_t n, uint64_t *out, uint32_t what);
 
 /* --- read-back (all synchronise) ---------------------------------------------------------------*/
+/* The spins S_i of PAPER.md:35 (stored 0..q-1), site i = y*L + x: the state of the chain after the last sweep (or as
+ * set by sw_init / sw_set_state).  SW_ERR_STATE before any of those.                                                */
 int sw_get_spins(sw_ctx *ctx, uint8_t *dst /* host [L*L] */);
 /* canonical roots of the LAST sweep; SW_ERR_STATE if there was none since sw_init */
 int sw_get_labels(sw_ctx *ctx, uint32_t *dst /* host [L*L] */);
 /* bonds of the LAST sweep, one byte per site (bit0 right, bit1 down); SW_ERR_STATE as above      */
 int sw_get_bonds(sw_ctx *ctx, uint8_t *dst /* host [L*L] */);
-/* rows y0 .. y0+nrows-1 only (for sampling a lattice too large to copy whole); what: 0 = spins
- * (uint8), 1 = labels (uint32), 2 = bonds (uint8)                                                */
+/* rows y0 .. y0+nrows-1 only of the same three arrays (spins PAPER.md:35, labels PAPER.md:42, bonds PAPER.md:40 step
+ * 1), for sampling a lattice too large to copy whole (2^32 sites: SURVEY.md sec. 8 c-6); what: 0 = spins (uint8),
+ * 1 = labels (uint32), 2 = bonds (uint8); dst: host, nrows*L elements; y0 + nrows <= L else SW_ERR_INVALID_ARG       */
 int sw_get_rows(sw_ctx *ctx, int what, uint32_t y0, uint32_t nrows, void *dst);
 int sw_get_threshold(sw_ctx *ctx, uint64_t *T);    /* floor((1-exp(-K)) * 2^32), 0..2^32          */
 int sw_get_time(sw_ctx *ctx, uint64_t *t);         /* sweeps done since sw_init (or set_state's t) */

@@ -599,7 +599,7 @@ int sw_sweep(sw_ctx *c, uint64_t n)
     DeviceGuard dg(c);
     if (c->cluster) {                    // small lattice: all the sweeps in one launch (chunks keep the 32-bit loop counter safe)
         for (uint64_t done = 0; done < n;) {
-            const uint64_t m = std::min<uint64_t>(n - done, 1u << 20);
+            const uint64_t m = std::min<uint64_t>(n - done, 1u << 16);   // (a launch of 65 536 sweeps runs for about two seconds)
             const int rc = sweep_cluster(c, m, 0, nullptr);
             if (rc != SW_OK) return rc;
             done += m;
