@@ -15,11 +15,15 @@
 //     higher columns and three shift-and-mask steps towards lower columns;
 //   * a component of the block is flood-filled from its smallest unvisited site: vertical step,
 //     horizontal closure, until nothing new appears;
-//   * "which component is site j in" is kept bit-sliced in five plane registers.
+//   * "which component is site j in" is kept bit-sliced in plane registers, transposed into one slot
+//     nibble per site once all components are known.
 // Only the components of the blocks (about 0.2 per site at q = 2, K_c instead of 0.53 horizontal
-// runs per site) go through the shared-memory union-find, over the bonds that cross a block edge
-// (0.16 per site): first up-link of every component by plain store, the rest with an atomic minimum.
+// runs per site) go through the shared-memory union-find, whose nodes ARE those components, over the
+// bonds that cross a block edge (0.16 per site): first up-link of every component by plain store,
+// the rest with a native 32-bit atomic minimum.
 #pragma once
+
+#include <type_traits>
 
 #include "sw_common.cuh"
 #include "sw_tiled.cuh"
@@ -29,65 +33,67 @@ namespace sw {
 constexpr int kBlkThreads = 128;
 constexpr int kBlkSlots = 26;                 // components of an 8 x 4 block that can have a link: <= 20 border singles + 6 pairs
 constexpr int kBlkExtraCap = 32 * 11;         // per warp: <= 7 up-links + 4 left-links per thread go through atomics
-constexpr uint32_t kDecodeMul = (1u << 24) | (1u << 17) | (1u << 10) | (1u << 3);
+constexpr uint32_t kOffMask = 0x3FFFu;        // the byte-offset half of a node entry
 
+// The union-find of a tile runs over the COMPONENTS OF THE BLOCKS, not over sites: node (k, tid) = slot k of the block of
+// thread tid, at byte offset off = 512 k + 4 tid of node[][].  Its entry is (seed id << 16) | off of its PARENT (the
+// seed = smallest site of the component, as a tile-local id y * 64 + x); a root holds its own.  Entries are unique per
+// node and ordered like the seeds, so hooking the larger root under the smaller is one native 32-bit atomicMin, the
+// root of a tile-local component is its smallest site, and the upper half of a root's entry IS the label
+// of the component's other sites.
 struct BlkShared {
-    uint16_t parent[kTileSites];              // union-find over tile-local site ids (y * 64 + x): component seeds are linked; a site of
-                                              // the right column of a block points at its seed (the block on its right links to the site)
-    uint32_t list[kBlkSlots][kBlkThreads];    // per thread, slot k: component mask -> seed id | seed bit << 16 -> tile-local id of its root
-    uint16_t pub_bottom[8][kBlkThreads];      // seed id of the component of my bottom-row site c
-    uint32_t edge[kBlkThreads];               // what the blocks below / to the right need to know about a block: bits 0-7 down
-                                              // bonds of row 3, 8-15 right bonds of row 3, 16-19 right bonds of column 7,
-                                              // 20-22 down bonds of column 7 (rows 0-2)
+    uint32_t node[kBlkSlots][kBlkThreads];    // flood fill: component masks; then the entries (see above); rows >= kBlkBufSlot double as link buffer
+    uint4 pub[kBlkThreads];                   // what the blocks below / to the right need to know about my components:
+                                              //   .x  slots of my bottom row, nibble p(c) = 2 (c % 4) + c / 4 for column c
+                                              //   .y  byte r = 5-bit slot of my site (r, 7)
+                                              //   .z  bit p(c) = fifth slot bit of my bottom-row site c (blocks with > 16 components)
+    uint32_t edge[kBlkThreads];               // bits 0-7 down bonds of row 3, 8-15 right bonds of row 3, 16-19 right bonds of
+                                              // column 7, 20-22 down bonds of column 7 (rows 0-2)
     uint32_t n_extra[kBlkThreads / 32];
+    uint32_t five;                            // some block of the tile has more than 16 components (slots need a fifth bit)
 };
-// The links that need the atomic pass are buffered per warp in list slots kBlkBufSlot .. kBlkSlots-1, which are
+// The links that need the atomic pass are buffered per warp in node rows kBlkBufSlot .. kBlkSlots-1, which are
 // free unless some block of the tile has more than kBlkBufSlot components (then they are united unbuffered).
 constexpr int kBlkBufSlot = 14;
 static_assert((kBlkSlots - kBlkBufSlot) * kBlkThreads >= (kBlkThreads / 32) * kBlkExtraCap, "link buffer too small");
+static_assert(kBlkSlots * kBlkThreads * 4 <= (int)kOffMask + 1, "node offsets need 14 bits");
 
-// ---- union-find on 16-bit parents ------------------------------------------------------------------
-// Links point to smaller ids, plain stores only ever replace a link
-// by a link to an ancestor, hooks are an atomic minimum (here a CAS on the 32-bit word that holds the entry:
-// a plain 16-bit store to either half in between makes the CAS fail and retry).
-__device__ __forceinline__ uint32_t atomic_min_u16(uint16_t *base, uint32_t idx, uint32_t val)
+__device__ __forceinline__ uint32_t ld_node(const uint32_t *U, uint32_t off)
 {
-    uint32_t *w = reinterpret_cast<uint32_t *>(base) + (idx >> 1);
-    const uint32_t sh = (idx & 1u) << 4;
-    uint32_t old = *reinterpret_cast<volatile uint32_t *>(w);
-    while (true) {
-        const uint32_t cur = (old >> sh) & 0xFFFFu;
-        if (cur <= val) return cur;
-        const uint32_t got = atomicCAS(w, old, (old & ~(0xFFFFu << sh)) | (val << sh));
-        if (got == old) return cur;
-        old = got;
-    }
+    return *reinterpret_cast<const volatile uint32_t *>(reinterpret_cast<const char *>(U) + off);
+}
+__device__ __forceinline__ void st_node(uint32_t *U, uint32_t off, uint32_t e)
+{
+    *reinterpret_cast<volatile uint32_t *>(reinterpret_cast<char *>(U) + off) = e;
 }
 
-__device__ __forceinline__ void unite_s16(uint16_t *parent_, uint32_t a, uint32_t b)
+// Join the components of nodes a and b (byte offsets).  A node is named by its own entry value s (s & kOffMask is
+// where it lives); links point to smaller entries, plain stores only ever replace a link by a link to an ancestor,
+// hooks are an atomic minimum: if the word hit was no longer a root, the link it held is not lost, we carry on
+// uniting its old target (one pass over all links yields the complete partition).
+__device__ __forceinline__ void unite_nodes(uint32_t *U, uint32_t a, uint32_t b)
 {
-    volatile uint16_t *parent = parent_;
-    {   // two unconditional hops on both sides first (a root points at itself): most chases end here, branch-free
-        const uint32_t a1 = parent[a], b1 = parent[b];
-        const uint32_t a2 = parent[a1], b2 = parent[b1];
-        if (a2 != a1) parent[a] = (uint16_t)a2;
-        if (b2 != b1) parent[b] = (uint16_t)b2;
-        a = a2; b = b2;
+    uint32_t sa = ld_node(U, a), sb = ld_node(U, b);
+    {   // one more unconditional hop on both sides (a root points at itself): most chases end here, branch-free
+        const uint32_t na = ld_node(U, sa & kOffMask), nb = ld_node(U, sb & kOffMask);
+        if (na != sa) st_node(U, a, na);
+        if (nb != sb) st_node(U, b, nb);
+        sa = na; sb = nb;
     }
     while (true) {
-        uint32_t pa = parent[a], pb = parent[b];
-        while (pa != a || pb != b) {
-            const uint32_t ga = parent[pa], gb = parent[pb];
-            if (ga != pa) parent[a] = (uint16_t)ga;
-            if (gb != pb) parent[b] = (uint16_t)gb;
-            a = ga; b = gb;
-            pa = parent[a]; pb = parent[b];
+        uint32_t pa = ld_node(U, sa & kOffMask), pb = ld_node(U, sb & kOffMask);
+        while (pa != sa || pb != sb) {
+            const uint32_t ga = ld_node(U, pa & kOffMask), gb = ld_node(U, pb & kOffMask);
+            if (ga != pa) st_node(U, sa & kOffMask, ga);
+            if (gb != pb) st_node(U, sb & kOffMask, gb);
+            sa = ga; sb = gb;
+            pa = ld_node(U, sa & kOffMask); pb = ld_node(U, sb & kOffMask);
         }
-        if (a == b) return;
-        if (a < b) { const uint32_t t = a; a = b; b = t; }
-        const uint32_t old = atomic_min_u16(parent_, a, b);
-        if (old == a) return;
-        a = old;
+        if (sa == sb) return;
+        if (sa < sb) { const uint32_t t = sa; sa = sb; sb = t; }
+        const uint32_t old = atomicMin(reinterpret_cast<uint32_t *>(reinterpret_cast<char *>(U) + (sa & kOffMask)), sb);
+        if (old == sa) return;
+        sa = old;
     }
 }
 
@@ -102,21 +108,21 @@ __device__ __forceinline__ uint32_t hclose(uint32_t n, uint32_t A, uint32_t A2, 
     return n;
 }
 
-// the four plane bytes of block row r as one word (byte b = plane b)
-__device__ __forceinline__ uint32_t plane_row(uint32_t P0, uint32_t P1, uint32_t P2, uint32_t P3, uint32_t r)
+// bit c of an 8-bit column mask -> bit p(c) = 2 (c % 4) + c / 4 (the order of the slot nibbles of a row)
+__device__ __forceinline__ uint32_t perm8(uint32_t x)
 {
-    const uint32_t sel = r | ((4u + r) << 4);
-    return __byte_perm(__byte_perm(P0, P1, sel), __byte_perm(P2, P3, sel), 0x5410);
+    uint32_t t = (x & 0x0Fu) | ((x & 0xF0u) << 4);            // columns 0-3 in bits 0-3, columns 4-7 in bits 8-11
+    t = (t | (t << 2)) & 0x3333u;
+    t = (t | (t << 1)) & 0x5555u;
+    return (t | (t >> 7)) & 0xFFu;
 }
 
-// component slot of column c from the row words (W: planes 0-3, V: plane 4 of the row shifted left by 4)
-__device__ __forceinline__ uint32_t slot_of(uint32_t W, uint32_t V, uint32_t c)
+// exchange the bits of hi selected by m << s with the bits of lo selected by m (delta swap across two registers)
+__device__ __forceinline__ void delta_swap(uint32_t &lo, uint32_t &hi, uint32_t s, uint32_t m)
 {
-    return ((((W >> c) & 0x01010101u) | ((V >> c) & 0x10u)) * kDecodeMul) >> 24;
-}
-__device__ __forceinline__ uint32_t slot_of4(uint32_t W, uint32_t c)
-{
-    return (((W >> c) & 0x01010101u) * kDecodeMul) >> 24;
+    const uint32_t t = ((lo >> s) ^ hi) & m;
+    hi ^= t;
+    lo ^= t << s;
 }
 
 // The body of the tile kernel for tile (tx, ty) of a piece of the lattice, run by kBlkThreads threads.
@@ -142,17 +148,11 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
     const uint32_t idbase = (by << 8) + (bx << 3);             // tile-local id of my first site
     const uint32_t i0 = origin + idbase / 64u * L + (bx << 3); // global index of my first site (mod 2^32 exact: N <= 2^32)
     const uint32_t a0 = kSuper ? y0 * W + x0 : i0;             // its array offset
+    const uint32_t tid4 = tid << 2;                            // byte offset of my column of node[][]
+    uint32_t *const U = &S.node[0][0];
 
-    // -- union-find array: identity
-    {
-        uint4 *p4 = reinterpret_cast<uint4 *>(S.parent);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const uint32_t e = (i * kBlkThreads + tid) * 8u, e2 = e * 0x00010001u + 0x00010000u;   // (e, e + 1) as two halves
-            p4[i * kBlkThreads + tid] = make_uint4(e2, e2 + 0x00020002u, e2 + 0x00040004u, e2 + 0x00060006u);
-        }
-        if (lane == 0) S.n_extra[warp] = 0;
-    }
+    if (tid < kBlkThreads / 32) S.n_extra[tid] = 0;
+    if (tid == 32) S.five = 0;
 
     // -- spins: my 4 rows of 8, the row below (from the lane 8 up, or from memory), the column to the right
     uint2 s[5];
@@ -228,7 +228,7 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
             bonds[(a0 + r * W) >> 4] = word;
         }
     }
-    Bar::sync();                                               // B1: parent[], edge[] visible
+    Bar::sync();                                               // B1: edge[], n_extra[], five visible
 
     // -- the bonds that leave the tile (warp 0): right bonds of block column 7, down bonds of block row 15
     if (warp == 0) {
@@ -270,65 +270,68 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
             if (v) {
                 m |= v;
             } else {
-                S.list[n][tid] = m;
+                S.node[n][tid] = m;
                 ++n;
                 rem &= ~m;
                 m = rem & (0u - rem);
             }
         }
     }
+    if (n > 16u) S.five = 1u;
 
-    // -- bit-sliced slot numbers (plane b holds bit b of the slot of every site) and the seed of every component
-    uint32_t P0 = 0, P1 = 0, P2 = 0, P3 = 0, P4 = 0;
+    // -- bit-sliced slot numbers (plane b holds bit b of the slot of every site); every component becomes a root node
+    uint32_t Q0 = 0, Q1 = 0, Q2 = 0, Q3 = 0, P4 = 0;
     {
         const uint32_t n_max = __reduce_max_sync(0xFFFFFFFFu, n);
 #pragma unroll
         for (int k = 0; k < kBlkSlots; ++k) {
             if ((uint32_t)k >= n_max) break;                  // warp-uniform
             if ((uint32_t)k < n) {
-                const uint32_t m = S.list[k][tid];
-                if (k & 1) P0 |= m;
-                if (k & 2) P1 |= m;
-                if (k & 4) P2 |= m;
-                if (k & 8) P3 |= m;
+                const uint32_t m = S.node[k][tid];
+                if (k & 1) Q0 |= m;
+                if (k & 2) Q1 |= m;
+                if (k & 4) Q2 |= m;
+                if (k & 8) Q3 |= m;
                 if (k & 16) P4 |= m;
                 const uint32_t j = __ffs(m) - 1u;
-                S.list[k][tid] = (idbase + ((j >> 3) << 6) + (j & 7u)) | (j << 16);
+                S.node[k][tid] = ((idbase + ((j >> 3) << 6) + (j & 7u)) << 16) | ((uint32_t)k * 512u + tid4);
             }
         }
     }
+    // planes 0-3 -> slot nibbles: afterwards nibble g of Q_i is the slot (mod 16) of site 4 g + i, i.e. of (r, c) with
+    // i = c % 4, g = 2 r + c / 4 (a 4 x 4 bit transpose across the four registers)
+    delta_swap(Q0, Q1, 1u, 0x55555555u);
+    delta_swap(Q2, Q3, 1u, 0x55555555u);
+    delta_swap(Q0, Q2, 2u, 0x33333333u);
+    delta_swap(Q1, Q3, 2u, 0x33333333u);
 
-    // -- publish the seeds of my bottom row for the block below (its up-links become plain-store parents); the sites
-    //    of my right column point at the seed of their component, and the block on my right links to those SITES
-    //    (one more hop in its finds; those links go through the atomic pass anyway)
+    // -- publish the slots of my bottom row and of my right column for the blocks below / to the right
     {
-        const uint32_t W3 = plane_row(P0, P1, P2, P3, 3u), V3 = (P4 >> 24) << 4;
-#pragma unroll
-        for (int c = 0; c < 8; ++c)
-            S.pub_bottom[c][tid] = (uint16_t)S.list[slot_of(W3, V3, c)][tid];
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const uint32_t Wr = plane_row(P0, P1, P2, P3, r), Vr = ((P4 >> (8 * r)) & 0xFFu) << 4;
-            if ((todo >> (8 * r + 7)) & 1u) S.parent[idbase + (r << 6) + 7u] = (uint16_t)S.list[slot_of(Wr, Vr, 7u)][tid];
-        }
+        const uint32_t bottom = __byte_perm(__byte_perm(Q0, Q1, 0x0073), __byte_perm(Q2, Q3, 0x0073), 0x5410);   // byte i = top byte of Q_i
+        const uint32_t col7 = ((Q3 >> 4) & 0x0F0F0F0Fu) | (((P4 >> 7) & 0x01010101u) << 4);
+        S.pub[tid] = make_uint4(bottom, col7, P4 ? perm8(P4 >> 24) : 0u, 0u);
     }
+    const uint32_t N0 = __byte_perm(__byte_perm(Q0, Q1, 0x0040), __byte_perm(Q2, Q3, 0x0040), 0x5410);           // slots of my row 0, nibble p(c)
 
     // -- links between blocks.  A link that repeats its neighbour's (same two components) is dropped.  The first
-    //    up-link of every component becomes its parent by plain store (the seed above is a smaller id, and a
+    //    up-link of every component becomes its parent by plain store (the component above has a smaller seed, and a
     //    component is written once: a forest); every other link needs the atomic pass after the barrier.
-    auto walk_links = [&](auto &&on_first, auto &&on_other) {
+    auto walk_links = [&](auto five_, auto &&on_first, auto &&on_other) {
+        constexpr bool kFive = decltype(five_)::value;
         if (up_row3) {
-            const uint32_t W0 = plane_row(P0, P1, P2, P3, 0u), V0 = (P4 & 0xFFu) << 4;
+            const uint4 pu = S.pub[tid - 8u];
             const uint32_t R_up = (e_up >> 8) & 0xFFu;
-            uint32_t u = up_row3 & ~((up_row3 & A & R_up & 0x7Fu) << 1);
+            uint32_t u = perm8(up_row3 & ~((up_row3 & A & R_up & 0x7Fu) << 1));
+            const uint32_t p4a = kFive ? perm8(P4 & 0xFFu) : 0u;
             uint32_t seen = 0;
             while (u) {
-                const uint32_t c = __ffs(u) - 1u;
+                const uint32_t p = __ffs(u) - 1u, sh = p << 2;
                 u &= u - 1u;
-                const uint32_t k = slot_of(W0, V0, c);
-                const uint32_t a = S.list[k][tid] & 0xFFFFu, b = S.pub_bottom[c][tid - 8u];
-                if (!((seen >> k) & 1u)) {
-                    seen |= 1u << k;
+                uint32_t ka = (N0 >> sh) & 15u, kb = (pu.x >> sh) & 15u;
+                if (kFive) { ka |= ((p4a >> p) & 1u) << 4; kb |= ((pu.z >> p) & 1u) << 4; }
+                const uint32_t a = (ka << 9) + tid4, b = (kb << 9) + tid4 - 32u;
+                if (!((seen >> ka) & 1u)) {
+                    seen |= 1u << ka;
                     on_first(a, b);
                 } else {
                     on_other(a, b);
@@ -336,74 +339,76 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
             }
         }
         if (left_c7) {
+            const uint32_t pl = S.pub[tid - 1u].y;
             const uint32_t D_left = (((e_left >> 20) & 7u) * 0x00204081u) & 0x00010101u;
             uint32_t l = left_c7 & ~((left_c7 & Dl & D_left) << 8);
             while (l) {
-                const uint32_t j = __ffs(l) - 1u, r = j >> 3;
+                const uint32_t j = __ffs(l) - 1u;              // = 8 r
                 l &= l - 1u;
-                const uint32_t Wr = plane_row(P0, P1, P2, P3, r), Vr = ((P4 >> j) & 0xFFu) << 4;
-                on_other(S.list[slot_of(Wr, Vr, 0u)][tid] & 0xFFFFu, idbase + (r << 6) - 1u);   // the site on my left
+                uint32_t ka = (Q0 >> j) & 15u;                 // site (r, 0) is nibble 2 r of Q0
+                if (kFive) ka |= ((P4 >> j) & 1u) << 4;
+                const uint32_t kb = (pl >> j) & 31u;
+                on_other((ka << 9) + tid4, (kb << 9) + tid4 - 4u);
             }
         }
     };
-    const bool crowded = Bar::sync_or(n > (uint32_t)kBlkBufSlot);   // B2: seeds of all blocks visible
-    uint32_t *const buf = &S.list[kBlkBufSlot][0] + warp * kBlkExtraCap;
+    const bool crowded = Bar::sync_or(n > (uint32_t)kBlkBufSlot);   // B2: the nodes and the published slots of all blocks visible
+    const bool five = S.five != 0u;
+    uint32_t *const buf = &S.node[kBlkBufSlot][0] + warp * kBlkExtraCap;
+    auto first = [&](uint32_t a, uint32_t b) { st_node(U, a, ld_node(U, b)); };   // b's entry, or already its parent's: an ancestor either way
     if (!crowded) {
-        walk_links([&](uint32_t a, uint32_t b) { S.parent[a] = (uint16_t)b; },
-                   [&](uint32_t a, uint32_t b) { buf[atomicAdd(&S.n_extra[warp], 1u)] = a | (b << 16); });
+        walk_links(std::false_type{}, first, [&](uint32_t a, uint32_t b) { buf[atomicAdd(&S.n_extra[warp], 1u)] = a | (b << 16); });
+    } else if (!five) {
+        walk_links(std::false_type{}, first, [](uint32_t, uint32_t) {});
     } else {
-        walk_links([&](uint32_t a, uint32_t b) { S.parent[a] = (uint16_t)b; }, [](uint32_t, uint32_t) {});
+        walk_links(std::true_type{}, first, [](uint32_t, uint32_t) {});
     }
     Bar::sync();                                               // B3: the plain-store forest is complete
     if (!crowded) {
         const uint32_t n_warp = S.n_extra[warp];
         for (uint32_t k = lane; k < n_warp; k += 32) {
             const uint32_t e = buf[k];
-            unite_s16(S.parent, e & 0xFFFFu, e >> 16);
+            unite_nodes(U, e & 0xFFFFu, e >> 16);
         }
+    } else if (!five) {
+        walk_links(std::false_type{}, [](uint32_t, uint32_t) {}, [&](uint32_t a, uint32_t b) { unite_nodes(U, a, b); });
     } else {
-        walk_links([](uint32_t, uint32_t) {}, [&](uint32_t a, uint32_t b) { unite_s16(S.parent, a, b); });
+        walk_links(std::true_type{}, [](uint32_t, uint32_t) {}, [&](uint32_t a, uint32_t b) { unite_nodes(U, a, b); });
     }
     Bar::sync();                                               // B4: no hooks happen any more
 
-    // -- every component: its root (chase; compress my own entry only) and root flag
+    // -- every component: its root (chase, then point my node straight at it: the labels below read it from there)
     uint32_t rootm = ~todo;                                    // a site without any bond is its own cluster
-    {
-        volatile uint16_t *par = S.parent;
-        for (uint32_t k = 0; k < n; ++k) {
-            const uint32_t e = S.list[k][tid], id = e & 0xFFFFu;
-            // three unconditional hops (a root points at itself, so hopping on is harmless), then the rare long chain
-            const uint32_t r1 = par[id], r2 = par[r1];
-            uint32_t r = r2, g = par[r2];
-            while (g != r) { r = g; g = par[r]; }
-            if (r != r1) par[id] = (uint16_t)r;
-            rootm |= (uint32_t)(r == id) << (e >> 16);
-            S.list[k][tid] = r;
-        }
+    for (uint32_t k = 0; k < n; ++k) {
+        const uint32_t off = (k << 9) + tid4;
+        // three unconditional hops (a root points at itself, so hopping on is harmless), then the rare long chain
+        const uint32_t r1 = ld_node(U, off), r2 = ld_node(U, r1 & kOffMask);
+        uint32_t r = r2, g = ld_node(U, r2 & kOffMask);
+        while (g != r) { r = g; g = ld_node(U, r & kOffMask); }
+        if (r != r1) st_node(U, off, r);
+        if ((r & kOffMask) == off) rootm |= 1u << (((r >> 19) & 24u) | ((r >> 16) & 7u));   // my seed (y * 64 + x): bit 8 (y % 4) + x % 8
     }
 
     // -- labels: a tile-local root keeps its own global index (the merge links it from there), every other site
-    //    gets the tile-local id of its root; root bitmap; roots of the edge sites as global indices for the merge
-    const bool five = __any_sync(0xFFFFFFFFu, n > 16u);
+    //    gets the tile-local id of its root (the upper half of its component's node); root bitmap; roots of the edge
+    //    sites as global indices for the merge
+    const bool five_w = __any_sync(0xFFFFFFFFu, n > 16u);      // (also reconverges the warp after the chases)
     auto global_of = [&](uint32_t v) { return origin + (v >> 6) * L + (v & 63u); };
+    const char *const mine = reinterpret_cast<const char *>(U) + tid4 + 2u;           // upper halves of my column of node[][]
     uint32_t col_l[4], col_r[4];
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
-        const uint32_t Wr = plane_row(P0, P1, P2, P3, r), Vr = ((P4 >> (8 * r)) & 0xFFu) << 4;
         const uint32_t self = i0 + r * L;
         uint32_t lab[8];
-        if (!five) {
 #pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                const uint32_t v = S.list[slot_of4(Wr, c)][tid];
-                lab[c] = ((rootm >> (8 * r + c)) & 1u) ? self + c : v;
-            }
-        } else {
-#pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                const uint32_t v = S.list[slot_of(Wr, Vr, c)][tid];
-                lab[c] = ((rootm >> (8 * r + c)) & 1u) ? self + c : v;
-            }
+        for (int c = 0; c < 8; ++c) {
+            const uint32_t Qi = (c & 3) == 0 ? Q0 : (c & 3) == 1 ? Q1 : (c & 3) == 2 ? Q2 : Q3;
+            const int sh = 4 * (2 * r + (c >> 2));                                    // my slot nibble sits at bit sh of Qi: * 512 = << 9
+            const uint32_t x = Qi & (0xFu << sh);
+            uint32_t o = sh <= 9 ? x << (9 - sh) : x >> (sh - 9);
+            if (five_w) o += ((P4 >> (8 * r + c)) & 1u) << 13;
+            const uint32_t v = *reinterpret_cast<const uint16_t *>(mine + o);
+            lab[c] = ((rootm >> (8 * r + c)) & 1u) ? self + c : v;
         }
         uint4 *lp = reinterpret_cast<uint4 *>(labels + (uint64_t)(y0 + r) * W + x0);
         lp[0] = make_uint4(lab[0], lab[1], lab[2], lab[3]);
