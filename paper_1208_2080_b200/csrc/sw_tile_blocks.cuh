@@ -33,11 +33,14 @@ namespace sw {
 constexpr int kBlkThreads = 128;
 constexpr int kBlkSlots = 26;                 // components of an 8 x 4 block that can have a link: <= 20 border singles + 6 pairs
 constexpr int kBlkExtraCap = 32 * 11;         // per warp: <= 7 up-links + 4 left-links per thread go through atomics
-constexpr uint32_t kOffMask = 0x3FFFu;        // the byte-offset half of a node entry
+constexpr uint32_t kOffMask = 0xFFFFu;        // the address half of a node entry
 
 // The union-find of a tile runs over the COMPONENTS OF THE BLOCKS, not over sites: node (k, tid) = slot k of the block of
-// thread tid, at byte offset off = 512 k + 4 tid of node[][].  Its entry is (seed id << 16) | off of its PARENT (the
-// seed = smallest site of the component, as a tile-local id y * 64 + x); a root holds its own.  Entries are unique per
+// thread tid, &node[k][tid].  Its entry is (seed id << 16) | the low 16 bits of the shared-memory address of its PARENT
+// (the seed = smallest site of the component, as a tile-local id y * 64 + x; static shared memory lies in the first
+// 64 KB of the CTA's window, so 16 bits hold the address and a hop is one logic instruction + one load; the upper
+// bits `win` of a shared address are the same for the whole CTA: zero, or the rank of the CTA in its cluster); a
+// root holds its own.  Entries are unique per
 // node and ordered like the seeds, so hooking the larger root under the smaller is one native 32-bit atomicMin, the
 // root of a tile-local component is its smallest site, and the upper half of a root's entry IS the label
 // of the component's other sites.
@@ -56,42 +59,70 @@ struct BlkShared {
 // free unless some block of the tile has more than kBlkBufSlot components (then they are united unbuffered).
 constexpr int kBlkBufSlot = 14;
 static_assert((kBlkSlots - kBlkBufSlot) * kBlkThreads >= (kBlkThreads / 32) * kBlkExtraCap, "link buffer too small");
-static_assert(kBlkSlots * kBlkThreads * 4 <= (int)kOffMask + 1, "node offsets need 14 bits");
 
-__device__ __forceinline__ uint32_t ld_node(const uint32_t *U, uint32_t off)
+// shared-memory accesses by 32-bit shared address (volatile: other threads hook and re-point nodes concurrently)
+__device__ __forceinline__ uint32_t ld_node(uint32_t addr)
 {
-    return *reinterpret_cast<const volatile uint32_t *>(reinterpret_cast<const char *>(U) + off);
+    uint32_t v;
+    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
 }
-__device__ __forceinline__ void st_node(uint32_t *U, uint32_t off, uint32_t e)
+__device__ __forceinline__ void st_node(uint32_t addr, uint32_t e)
 {
-    *reinterpret_cast<volatile uint32_t *>(reinterpret_cast<char *>(U) + off) = e;
+    asm volatile("st.volatile.shared.u32 [%0], %1;" :: "r"(addr), "r"(e) : "memory");
+}
+__device__ __forceinline__ uint32_t min_node(uint32_t addr, uint32_t e)
+{
+    uint32_t old;
+    asm volatile("atom.shared.min.u32 %0, [%1], %2;" : "=r"(old) : "r"(addr), "r"(e) : "memory");
+    return old;
+}
+// after the last hook: entries only ever change to the root's, either value ends the chase at the same root
+__device__ __forceinline__ uint32_t ld_node_quiet(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint32_t and_opaque(uint32_t a, uint32_t m)
+{
+    uint32_t v;
+    asm("and.b32 %0, %1, %2;" : "=r"(v) : "r"(a), "r"(m));
+    return v;
+}
+__device__ __forceinline__ uint32_t ld_label_half(uint32_t addr)
+{
+    uint16_t v;
+    asm volatile("ld.shared.u16 %0, [%1+2];" : "=h"(v) : "r"(addr) : "memory");
+    return v;
 }
 
-// Join the components of nodes a and b (byte offsets).  A node is named by its own entry value s (s & kOffMask is
+// Join the components of nodes a and b (shared-memory addresses).  A node is named by its own entry value s (s & kOffMask is
 // where it lives); links point to smaller entries, plain stores only ever replace a link by a link to an ancestor,
 // hooks are an atomic minimum: if the word hit was no longer a root, the link it held is not lost, we carry on
 // uniting its old target (one pass over all links yields the complete partition).
-__device__ __forceinline__ void unite_nodes(uint32_t *U, uint32_t a, uint32_t b)
+__device__ __forceinline__ void unite_nodes(uint32_t a, uint32_t b, const uint32_t win)
 {
-    uint32_t sa = ld_node(U, a), sb = ld_node(U, b);
+    auto at = [win](uint32_t e) { return (e & kOffMask) | win; };     // where the node named by entry e lives
+    uint32_t sa = ld_node(a), sb = ld_node(b);
     {   // one more unconditional hop on both sides (a root points at itself): most chases end here, branch-free
-        const uint32_t na = ld_node(U, sa & kOffMask), nb = ld_node(U, sb & kOffMask);
-        if (na != sa) st_node(U, a, na);
-        if (nb != sb) st_node(U, b, nb);
+        const uint32_t na = ld_node(at(sa)), nb = ld_node(at(sb));
+        if (na != sa) st_node(a, na);
+        if (nb != sb) st_node(b, nb);
         sa = na; sb = nb;
     }
     while (true) {
-        uint32_t pa = ld_node(U, sa & kOffMask), pb = ld_node(U, sb & kOffMask);
+        uint32_t pa = ld_node(at(sa)), pb = ld_node(at(sb));
         while (pa != sa || pb != sb) {
-            const uint32_t ga = ld_node(U, pa & kOffMask), gb = ld_node(U, pb & kOffMask);
-            if (ga != pa) st_node(U, sa & kOffMask, ga);
-            if (gb != pb) st_node(U, sb & kOffMask, gb);
+            const uint32_t ga = ld_node(at(pa)), gb = ld_node(at(pb));
+            if (ga != pa) st_node(at(sa), ga);
+            if (gb != pb) st_node(at(sb), gb);
             sa = ga; sb = gb;
-            pa = ld_node(U, sa & kOffMask); pb = ld_node(U, sb & kOffMask);
+            pa = ld_node(at(sa)); pb = ld_node(at(sb));
         }
         if (sa == sb) return;
         if (sa < sb) { const uint32_t t = sa; sa = sb; sb = t; }
-        const uint32_t old = atomicMin(reinterpret_cast<uint32_t *>(reinterpret_cast<char *>(U) + (sa & kOffMask)), sb);
+        const uint32_t old = min_node(at(sa), sb);
         if (old == sa) return;
         sa = old;
     }
@@ -148,8 +179,9 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
     const uint32_t idbase = (by << 8) + (bx << 3);             // tile-local id of my first site
     const uint32_t i0 = origin + idbase / 64u * L + (bx << 3); // global index of my first site (mod 2^32 exact: N <= 2^32)
     const uint32_t a0 = kSuper ? y0 * W + x0 : i0;             // its array offset
-    const uint32_t tid4 = tid << 2;                            // byte offset of my column of node[][]
-    uint32_t *const U = &S.node[0][0];
+    const uint32_t mybase = (uint32_t)__cvta_generic_to_shared(&S.node[0][tid]);   // shared address of my column of node[][]
+    // its window bits (only a CTA of a multi-CTA cluster has any: the kCoherent instantiation) / its 16 address bits in an entry
+    const uint32_t win = kCoherent ? mybase & ~kOffMask : 0u, my16 = mybase & kOffMask;
 
     if (tid < kBlkThreads / 32) S.n_extra[tid] = 0;
     if (tid == 32) S.five = 0;
@@ -294,7 +326,7 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
                 if (k & 8) Q3 |= m;
                 if (k & 16) P4 |= m;
                 const uint32_t j = __ffs(m) - 1u;
-                S.node[k][tid] = ((idbase + ((j >> 3) << 6) + (j & 7u)) << 16) | ((uint32_t)k * 512u + tid4);
+                S.node[k][tid] = ((idbase + ((j >> 3) << 6) + (j & 7u)) << 16) + ((uint32_t)k * 512u + my16);
             }
         }
     }
@@ -329,7 +361,7 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
                 u &= u - 1u;
                 uint32_t ka = (N0 >> sh) & 15u, kb = (pu.x >> sh) & 15u;
                 if (kFive) { ka |= ((p4a >> p) & 1u) << 4; kb |= ((pu.z >> p) & 1u) << 4; }
-                const uint32_t a = (ka << 9) + tid4, b = (kb << 9) + tid4 - 32u;
+                const uint32_t a = (ka << 9) + mybase, b = (kb << 9) + mybase - 32u;
                 if (!((seen >> ka) & 1u)) {
                     seen |= 1u << ka;
                     on_first(a, b);
@@ -348,16 +380,16 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
                 uint32_t ka = (Q0 >> j) & 15u;                 // site (r, 0) is nibble 2 r of Q0
                 if (kFive) ka |= ((P4 >> j) & 1u) << 4;
                 const uint32_t kb = (pl >> j) & 31u;
-                on_other((ka << 9) + tid4, (kb << 9) + tid4 - 4u);
+                on_other((ka << 9) + mybase, (kb << 9) + mybase - 4u);
             }
         }
     };
     const bool crowded = Bar::sync_or(n > (uint32_t)kBlkBufSlot);   // B2: the nodes and the published slots of all blocks visible
     const bool five = S.five != 0u;
     uint32_t *const buf = &S.node[kBlkBufSlot][0] + warp * kBlkExtraCap;
-    auto first = [&](uint32_t a, uint32_t b) { st_node(U, a, ld_node(U, b)); };   // b's entry, or already its parent's: an ancestor either way
+    auto first = [&](uint32_t a, uint32_t b) { st_node(a, ld_node(b)); };   // b's entry, or already its parent's: an ancestor either way
     if (!crowded) {
-        walk_links(std::false_type{}, first, [&](uint32_t a, uint32_t b) { buf[atomicAdd(&S.n_extra[warp], 1u)] = a | (b << 16); });
+        walk_links(std::false_type{}, first, [&](uint32_t a, uint32_t b) { buf[atomicAdd(&S.n_extra[warp], 1u)] = (a & kOffMask) | (b << 16); });
     } else if (!five) {
         walk_links(std::false_type{}, first, [](uint32_t, uint32_t) {});
     } else {
@@ -368,25 +400,26 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
         const uint32_t n_warp = S.n_extra[warp];
         for (uint32_t k = lane; k < n_warp; k += 32) {
             const uint32_t e = buf[k];
-            unite_nodes(U, e & 0xFFFFu, e >> 16);
+            unite_nodes((e & kOffMask) | win, (e >> 16) | win, win);
         }
     } else if (!five) {
-        walk_links(std::false_type{}, [](uint32_t, uint32_t) {}, [&](uint32_t a, uint32_t b) { unite_nodes(U, a, b); });
+        walk_links(std::false_type{}, [](uint32_t, uint32_t) {}, [&](uint32_t a, uint32_t b) { unite_nodes(a, b, win); });
     } else {
-        walk_links(std::true_type{}, [](uint32_t, uint32_t) {}, [&](uint32_t a, uint32_t b) { unite_nodes(U, a, b); });
+        walk_links(std::true_type{}, [](uint32_t, uint32_t) {}, [&](uint32_t a, uint32_t b) { unite_nodes(a, b, win); });
     }
     Bar::sync();                                               // B4: no hooks happen any more
 
     // -- every component: its root (chase, then point my node straight at it: the labels below read it from there)
     uint32_t rootm = ~todo;                                    // a site without any bond is its own cluster
     for (uint32_t k = 0; k < n; ++k) {
-        const uint32_t off = (k << 9) + tid4;
+        const uint32_t me = (k << 9) + mybase;
+        auto at = [win](uint32_t e) { return (e & kOffMask) | win; };
         // three unconditional hops (a root points at itself, so hopping on is harmless), then the rare long chain
-        const uint32_t r1 = ld_node(U, off), r2 = ld_node(U, r1 & kOffMask);
-        uint32_t r = r2, g = ld_node(U, r2 & kOffMask);
-        while (g != r) { r = g; g = ld_node(U, r & kOffMask); }
-        if (r != r1) st_node(U, off, r);
-        if ((r & kOffMask) == off) rootm |= 1u << (((r >> 19) & 24u) | ((r >> 16) & 7u));   // my seed (y * 64 + x): bit 8 (y % 4) + x % 8
+        const uint32_t r1 = ld_node_quiet(me), r2 = ld_node_quiet(at(r1));
+        uint32_t r = r2, g = ld_node_quiet(at(r2));
+        while (g != r) { r = g; g = ld_node_quiet(at(r)); }
+        if (r != r1) st_node(me, r);
+        if (at(r) == me) rootm |= 1u << (((r >> 19) & 24u) | ((r >> 16) & 7u));   // my seed (y * 64 + x): bit 8 (y % 4) + x % 8
     }
 
     // -- labels: a tile-local root keeps its own global index (the merge links it from there), every other site
@@ -394,36 +427,44 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
     //    sites as global indices for the merge
     const bool five_w = __any_sync(0xFFFFFFFFu, n > 16u);      // (also reconverges the warp after the chases)
     auto global_of = [&](uint32_t v) { return origin + (v >> 6) * L + (v & 63u); };
-    const char *const mine = reinterpret_cast<const char *>(U) + tid4 + 2u;           // upper halves of my column of node[][]
     uint32_t col_l[4], col_r[4];
+    auto write_labels = [&](auto five_) {
+        constexpr bool kFive = decltype(five_)::value;
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
-        const uint32_t self = i0 + r * L;
-        uint32_t lab[8];
+        for (int r = 0; r < 4; ++r) {
+            const uint32_t self = i0 + r * L, rb = __byte_perm(rootm, 0, 0x4440 + r);
+            uint32_t lab[8];
 #pragma unroll
-        for (int c = 0; c < 8; ++c) {
-            const uint32_t Qi = (c & 3) == 0 ? Q0 : (c & 3) == 1 ? Q1 : (c & 3) == 2 ? Q2 : Q3;
-            const int sh = 4 * (2 * r + (c >> 2));                                    // my slot nibble sits at bit sh of Qi: * 512 = << 9
-            const uint32_t x = Qi & (0xFu << sh);
-            uint32_t o = sh <= 9 ? x << (9 - sh) : x >> (sh - 9);
-            if (five_w) o += ((P4 >> (8 * r + c)) & 1u) << 13;
-            const uint32_t v = *reinterpret_cast<const uint16_t *>(mine + o);
-            lab[c] = ((rootm >> (8 * r + c)) & 1u) ? self + c : v;
+            for (int c = 0; c < 8; ++c) {
+                // my slot nibble sits at bit sh of Q_(c % 4); * 512 = the row of node[][].  (The AND is opaque to the
+                // compiler so that it stays in front of the shift: mask, then one shift-and-add.)
+                const uint32_t Qi = (c & 3) == 0 ? Q0 : (c & 3) == 1 ? Q1 : (c & 3) == 2 ? Q2 : Q3;
+                constexpr int kZero = 0;
+                const int sh = 4 * (2 * r + (c >> 2)) + kZero;
+                const uint32_t x = and_opaque(Qi, 0xFu << sh);
+                uint32_t o = mybase + (sh <= 9 ? x << (9 - sh) : x >> (sh - 9));
+                if (kFive) o += ((P4 >> (8 * r + c)) & 1u) << 13;
+                uint32_t v = ld_label_half(o);
+                if (rb & (1u << c)) v = self + c;
+                lab[c] = v;
+            }
+            uint4 *lp = reinterpret_cast<uint4 *>(labels + (uint64_t)(y0 + r) * W + x0);
+            lp[0] = make_uint4(lab[0], lab[1], lab[2], lab[3]);
+            lp[1] = make_uint4(lab[4], lab[5], lab[6], lab[7]);
+            col_l[r] = lab[0];
+            col_r[r] = lab[7];
+            if ((r == 0 && by == 0u) || (r == 3 && by == 15u)) {   // top / bottom row of the tile
+                uint32_t g[8];
+#pragma unroll
+                for (int c = 0; c < 8; ++c) g[c] = ((rootm >> (8 * r + c)) & 1u) ? lab[c] : global_of(lab[c]);
+                uint4 *ep = reinterpret_cast<uint4 *>((r == 0 ? edges[tile].top : edges[tile].bottom) + 8u * bx);
+                ep[0] = make_uint4(g[0], g[1], g[2], g[3]);
+                ep[1] = make_uint4(g[4], g[5], g[6], g[7]);
+            }
         }
-        uint4 *lp = reinterpret_cast<uint4 *>(labels + (uint64_t)(y0 + r) * W + x0);
-        lp[0] = make_uint4(lab[0], lab[1], lab[2], lab[3]);
-        lp[1] = make_uint4(lab[4], lab[5], lab[6], lab[7]);
-        col_l[r] = lab[0];
-        col_r[r] = lab[7];
-        if ((r == 0 && by == 0u) || (r == 3 && by == 15u)) {   // top / bottom row of the tile
-            uint32_t g[8];
-#pragma unroll
-            for (int c = 0; c < 8; ++c) g[c] = ((rootm >> (8 * r + c)) & 1u) ? lab[c] : global_of(lab[c]);
-            uint4 *ep = reinterpret_cast<uint4 *>((r == 0 ? edges[tile].top : edges[tile].bottom) + 8u * bx);
-            ep[0] = make_uint4(g[0], g[1], g[2], g[3]);
-            ep[1] = make_uint4(g[4], g[5], g[6], g[7]);
-        }
-    }
+    };
+    if (!five_w) write_labels(std::false_type{});
+    else write_labels(std::true_type{});
     {
         const uint32_t pm = __shfl_xor_sync(0xFFFFFFFFu, rootm, 1);
         const uint32_t me = odd ? pm : rootm, mo = odd ? rootm : pm;
