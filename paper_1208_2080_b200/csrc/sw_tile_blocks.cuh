@@ -491,7 +491,10 @@ struct CtaBar {
     static __device__ __forceinline__ bool sync_or(bool p) { return __syncthreads_or(p) != 0; }
 };
 
-__global__ void __launch_bounds__(kBlkThreads, 9)
+#ifndef SW_BLK_CTAS
+#define SW_BLK_CTAS 12
+#endif
+__global__ void __launch_bounds__(kBlkThreads, SW_BLK_CTAS)
 k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
               uint32_t *__restrict__ labels, uint16_t *__restrict__ rootbits,
               TileBorder *__restrict__ border, TileEdges *__restrict__ edges, const uint2 *__restrict__ draws, Params P)
