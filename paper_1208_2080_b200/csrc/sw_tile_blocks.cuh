@@ -504,7 +504,7 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
 }
 
 // the same for one sub-lattice of the super-lattice (sw_super.cu); grid = (W / 64, H / 64)
-__global__ void __launch_bounds__(kBlkThreads, 9)
+__global__ void __launch_bounds__(kBlkThreads, SW_BLK_CTAS)
 k_tile_blocks_super(const uint8_t *spins, uint32_t *__restrict__ bonds,
                     uint32_t *__restrict__ labels, uint16_t *__restrict__ rootbits,
                     TileBorder *__restrict__ border, TileEdges *__restrict__ edges, const uint2 *__restrict__ draws, Params P, Dom dom)

@@ -276,19 +276,22 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
     //    it), so the first step of every chase comes out of this coalesced load instead of a scattered one.
     //    What a site needs afterwards is the tile-local id of its root (12 bits; its own id if it is a root): two per
     //    register, so the 16 sites of a thread cost 8 registers across the chases instead of 16.
-    uint32_t ids[2 * kAcc];
     uint32_t work = 0;                                         // bit 4k + j: my site j of access k is a tile-local root
-    uint4 lq[kAcc];
     uint32_t rq[kAcc];
     if (kSizes) {
         for (uint32_t k = tid; k < kTileSites; k += NT) Z->cnt[k] = 0;
         if (tid < kTileSites / 32) Z->touch[tid] = 0;
         Bar::sync();
     }
+    // The labels go straight to shared memory (cp.async, L2 only: 16 bytes per thread and access, no registers held
+    // while they are in flight): a root's entry is where its chase starts (and is replaced by the canonical root
+    // below), every other site's entry keeps the tile-local id of its root until phase C reads it back -- nothing
+    // per site has to stay in registers across the draws and the chases.
 #pragma unroll
     for (int k = 0; k < kAcc; ++k) {
-        const uint32_t o = a00 + 2 * k * W;
-        lq[k] = __ldcg(reinterpret_cast<const uint4 *>(labels + o));
+        const uint32_t o = a00 + 2 * k * W, id0 = ((yk0 + 2 * k) << 6) + x4;
+        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&S.root[id0]);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(dst), "l"(labels + o) : "memory");
         rq[k] = rootbits[o >> 4];
     }
     // while those loads are on their way: the bond draws of the NEXT sweep for this tile (pure arithmetic, see above)
@@ -297,26 +300,21 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
         for (int u = 0; u < 256; u += NT) tile_draw_masks(next_draws, tile, origin, tid + u, pk_n, P, L);
     }
 #pragma unroll
-    for (int k = 0; k < kAcc; ++k) {
-        const uint4 l = lq[k];
-        const uint32_t lab[4] = {l.x, l.y, l.z, l.w};
-        const uint32_t rb = (rq[k] >> (x4 & 12u)) & 15u;
-        const uint32_t id0 = ((yk0 + 2 * k) << 6) + x4;
-        // where the chase of a root starts: its own entry.  All four entries are stored with one 16-byte store; the
-        // entries of sites that are not roots are never read (every lookup goes to a root's id).
-        *reinterpret_cast<uint4 *>(&S.root[id0]) = l;
-        uint32_t id[4];
+    for (int k = 0; k < kAcc; ++k) work |= ((rq[k] >> (x4 & 12u)) & 15u) << (4 * k);
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    if (kSizes) {                                              // border sites of the tile mark their root
 #pragma unroll
-        for (int j = 0; j < 4; ++j) id[j] = ((rb >> j) & 1u) ? id0 + j : lab[j];
-        ids[2 * k] = id[0] | (id[1] << 16);
-        ids[2 * k + 1] = id[2] | (id[3] << 16);
-        work |= rb << (4 * k);
-        if (kSizes) {                                          // border sites of the tile mark their root
+        for (int k = 0; k < kAcc; ++k) {
+            const uint32_t id0 = ((yk0 + 2 * k) << 6) + x4, rb = (work >> (4 * k)) & 15u;
+            const uint4 l = *reinterpret_cast<const uint4 *>(&S.root[id0]);
+            const uint32_t lab[4] = {l.x, l.y, l.z, l.w};
             const uint32_t y = yk0 + 2 * k;
             const bool row_edge = y == 0 || y + 1 == kTile;
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
-                if (row_edge || x4 + j == 0 || x4 + j + 1 == kTile) atomicOr(&Z->touch[id[j] >> 5], 1u << (id[j] & 31u));
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t id = ((rb >> j) & 1u) ? id0 + j : lab[j];
+                if (row_edge || x4 + j == 0 || x4 + j + 1 == kTile) atomicOr(&Z->touch[id >> 5], 1u << (id & 31u));
+            }
         }
     }
 
@@ -372,10 +370,17 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
 #pragma unroll
     for (int k = 0; k < kAcc; ++k) {
         const uint32_t i0 = i00 + 2 * k * L, o = a00 + 2 * k * W;
-        uint32_t st = 0, lab[4];
+        uint32_t st = 0, lab[4], qid[4];
+        {
+            const uint32_t id0 = ((yk0 + 2 * k) << 6) + x4, rb = (work >> (4 * k)) & 15u;
+            const uint4 l = *reinterpret_cast<const uint4 *>(&S.root[id0]);           // my own entries, as phase A left them
+            const uint32_t mine[4] = {l.x, l.y, l.z, l.w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) qid[j] = ((rb >> j) & 1u) ? id0 + j : mine[j];
+        }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const uint32_t id = (j & 1) ? ids[2 * k + (j >> 1)] >> 16 : ids[2 * k + (j >> 1)] & 0xFFFFu;
+            const uint32_t id = qid[j];
             lab[j] = S.root[id];
             if (kCount) canon += (lab[j] == i0 + j);           // a canonical root is its own label
             if (kSpins) st |= (uint32_t)S.state[id] << (8 * j);
@@ -383,7 +388,6 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
         if (kSizes) {
             // my 4 sites count for their tile-local roots, runs of equal ids together; a root does not count itself (it is
             // added when the counts are read), so singletons -- a quarter of the sites at q = 10 -- cost no atomic at all
-            const uint32_t qid[4] = {ids[2 * k] & 0xFFFFu, ids[2 * k] >> 16, ids[2 * k + 1] & 0xFFFFu, ids[2 * k + 1] >> 16};
             const uint32_t rb = (work >> (4 * k)) & 15u;
             uint32_t cur = qid[0], len = (rb & 1u) ^ 1u;
 #pragma unroll
@@ -416,8 +420,11 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
     }
 }
 
+#ifndef SW_FLIP_CTAS
+#define SW_FLIP_CTAS 7
+#endif
 template <bool kLabels, bool kSpins, bool kCount, bool kStats = false>
-__global__ void __launch_bounds__(kFlipThreads, 6)
+__global__ void __launch_bounds__(kFlipThreads, SW_FLIP_CTAS)
 k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__restrict__ spins, Params P,
             uint32_t *__restrict__ tile_clusters, uint2 *__restrict__ next_draws, PassCounters *__restrict__ counters = nullptr)
 {
@@ -441,7 +448,7 @@ k_tile_flip_sizes(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8
 // one sub-lattice of the super-lattice; grid = (W / 64, H / 64).  `spins` is read by the neighbours' tile kernels of the
 // next sweep (their halo), never by this kernel.
 template <bool kLabels, bool kSpins, bool kCount>
-__global__ void __launch_bounds__(kFlipThreads, 6)
+__global__ void __launch_bounds__(kFlipThreads, SW_FLIP_CTAS)
 k_tile_flip_super(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *spins, Params P, Dom dom,
                   uint32_t *__restrict__ tile_clusters, uint2 *__restrict__ next_draws)
 {
