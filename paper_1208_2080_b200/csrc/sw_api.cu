@@ -35,7 +35,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Plan {
-    size_t spins, bonds, labels, rootbits, border, edges, tile_clusters, draws, row, flag, rows, stage, counters, sizes, total;   // byte offsets into the workspace
+    size_t spins, bonds, labels, rootbits, border, edges, btab, tile_clusters, draws, row, flag, rows, stage, counters, sizes, total;   // byte offsets into the workspace
     size_t rows_cap, stage_bytes;      // rows of the sw_sweep_measure ring; bytes of the sw_get_bonds staging buffer
 };
 
@@ -55,6 +55,7 @@ Plan make_plan(uint32_t L, uint32_t q, uint32_t flags)
     p.rootbits = off; off = align_up(off + (tiled_ok(L, flags) ? (N / 16) * 2 : 0));
     p.border = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileBorder) : 0));
     p.edges = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sizeof(sw::TileEdges) : 0));
+    p.btab = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * sw::kBorderTabEntries * 4 : 0));
     p.tile_clusters = off; off = align_up(off + (tiled_ok(L, flags) ? (N / sw::kTileSites) * (sw::kFlipThreads / 32) * 4 : 0));
     p.draws = off;  off = align_up(off + (tiled_ok(L, flags) ? (N / 32) * sizeof(uint2) : 0));   // one uint2 per 8 x 4 block
     p.row = off;    off = align_up(off + (3 + (size_t)q + 2) * 8);   // + the two words of sum |c|^2 (sw_measure_clusters)
@@ -96,6 +97,7 @@ struct sw_ctx {
     uint16_t *d_rootbits = nullptr;
     sw::TileBorder *d_border = nullptr;
     sw::TileEdges *d_edges = nullptr;
+    uint32_t *d_btab = nullptr;          // per tile: the components that own a site on the tile border (k_tile_blocks_sizes)
     unsigned long long *d_row = nullptr;
     unsigned long long *d_rows = nullptr; // ring of observable rows for sw_sweep_measure (rows_cap rows)
     size_t rows_cap = 0;
@@ -105,8 +107,8 @@ struct sw_ctx {
     bool count_passes = false;
     uint32_t *d_sizes = nullptr;          // 4N-byte scratch for cluster sizes: in the workspace (SW_FLAG_WS_CLUSTER_SIZES) or
     bool owns_sizes = false;              // allocated once by the first sw_measure(largest_cluster)
-    bool sizes_zero = false;              // d_sizes is all zero (k_max_size_zero leaves it so; k_tile_flip_sizes relies on it)
-    uint64_t sizes_t = ~0ull;             // == t: d_sizes holds the cluster sizes of the last sweep, counted by k_tile_flip_sizes
+    bool sizes_zero = false;              // d_sizes is all zero (k_max_size_zero leaves it so; the counting sweeps rely on it)
+    uint64_t sizes_t = ~0ull;             // == t: d_sizes holds the cluster sizes of the last sweep, counted by k_tile_blocks_sizes + k_tile_flip_sizes
     uint64_t launches = 0, sweeps = 0;
     int num_sms = 148;
     // profiling: events are created once and reused (no cudaEventCreate inside a timed region after the first pass)
@@ -261,8 +263,10 @@ int ensure_sizes_zero(sw_ctx *c)
 }
 
 // count_clusters: the flip kernel also counts the canonical roots (wanted for the last sweep before a measurement);
-// sizes_row != nullptr (a zeroed row of observables): it counts the cluster sizes as well (k_tile_flip_sizes) and raises
-// sizes_row[2] to the largest cluster that lies inside one tile; the rest is in d_sizes for k_max_size_zero
+// sizes_row != nullptr (a zeroed row of observables): the sweep counts the cluster sizes as well.  The tile kernel counts
+// the sites of its tile-local components: those inside one tile are whole clusters and only raise sizes_row[2], the
+// others go through the tile's border table to the flip kernel, which adds them up in d_sizes at the canonical roots for
+// k_max_size_zero (k_tile_blocks_sizes, k_tile_flip_sizes)
 int sweep_once(sw_ctx *c, bool count_clusters, unsigned long long *sizes_row = nullptr)
 {
     const Params P = make_params(c, c->t);
@@ -273,18 +277,22 @@ int sweep_once(sw_ctx *c, bool count_clusters, unsigned long long *sizes_row = n
             c->launches += 1;
             sw::k_draws<<<tgrid, 256, 0, c->stream>>>(c->d_draws, P);
         }
+        const bool with_sizes = sizes_row && !c->lazy && !c->count_passes;
+        if (with_sizes) {
+            const int rc = ensure_sizes_zero(c);
+            if (rc != SW_OK) return rc;
+            Timed tm(c, SLOT_TILE);
+            sw::k_tile_blocks_sizes<<<tgrid, sw::kBlkThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_edges, c->d_draws, P, c->d_btab, sizes_row);
+            c->sizes_zero = false;
+        } else
         { Timed tm(c, SLOT_TILE);
           sw::k_tile_blocks<<<tgrid, sw::kBlkThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_edges, c->d_draws, P); }
         { Timed tm(c, SLOT_MERGE);
           auto merge = c->count_passes ? sw::k_tile_merge<true> : sw::k_tile_merge<false>;
           merge<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_edges, P, tiles, c->d_counters); }
-        const bool with_sizes = sizes_row && !c->lazy && !c->count_passes;
         if (with_sizes) {
-            const int rc = ensure_sizes_zero(c);
-            if (rc != SW_OK) return rc;
             Timed tm(c, SLOT_FLIP);
-            sw::k_tile_flip_sizes<<<tgrid, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, c->d_draws, c->d_sizes, sizes_row);
-            c->sizes_zero = false;
+            sw::k_tile_flip_sizes<<<tgrid, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, c->d_draws, c->d_sizes, c->d_btab);
             c->sizes_t = c->t + 1;
         } else
         { Timed tm(c, SLOT_FLIP);
@@ -355,7 +363,7 @@ int ensure_flat(sw_ctx *c)
 }
 
 // Enqueue the observable kernels for the current state into the device row `row` (zeroed here).
-// row_is_zero: the caller zeroed the row already (and k_tile_flip_sizes may have put the largest tile-local cluster into row[2])
+// row_is_zero: the caller zeroed the row already
 int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m, bool want_nc, bool want_big, unsigned long long *c2 = nullptr,
                     bool row_is_zero = false)
 {
@@ -377,7 +385,7 @@ int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m
             sw::k_observe_scalar<<<grid_for(c, c->N, sw::kObsThreads), sw::kObsThreads, 0, c->stream>>>(c->d_spins, c->d_labels, P, want, row);
     }
     if (cl && want_big && c->tiled && c->sizes_t == c->t && !c2) {
-        // the flip kernel of the last sweep counted the sizes: clusters inside one tile are in row[2] already, the others in d_sizes
+        // the kernels of the last sweep counted the sizes: clusters inside one tile are in row[2] already, the others in d_sizes
         c->launches += 1;
         sw::k_max_size_zero<<<grid_for(c, c->N / 4, 256), 256, 0, c->stream>>>(c->d_sizes, P, row);
         c->sizes_zero = true;
@@ -446,6 +454,7 @@ int create_common(sw_ctx **out, uint32_t L, uint32_t q, double K, uint64_t seed,
     c->d_rootbits = (uint16_t *)(c->ws + plan.rootbits);
     c->d_border = (sw::TileBorder *)(c->ws + plan.border);
     c->d_edges = (sw::TileEdges *)(c->ws + plan.edges);
+    c->d_btab = (uint32_t *)(c->ws + plan.btab);
     c->d_tile_clusters = (uint32_t *)(c->ws + plan.tile_clusters);
     c->d_draws = (uint2 *)(c->ws + plan.draws);
     c->d_row = (unsigned long long *)(c->ws + plan.row);

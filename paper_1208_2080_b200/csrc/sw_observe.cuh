@@ -189,11 +189,12 @@ __global__ void k_max_size(const uint32_t *__restrict__ sizes, Params P, unsigne
 }
 
 // the same, and every counter that was read non-zero is set back to zero: sizes[] stays all zero between measurements
-// (k_tile_flip_sizes relies on that), without a memset of 4N bytes per measurement
+// (the counting sweeps rely on that), without a memset of 4N bytes per measurement.  A site without any bond is a
+// cluster of one whose counter may have been left at zero (k_tile_blocks_sizes): the maximum is at least 1.
 __global__ void k_max_size_zero(uint32_t *__restrict__ sizes, Params P, unsigned long long *row)
 {
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x * 4;
-    uint32_t m = 0;
+    uint32_t m = (blockIdx.x == 0 && threadIdx.x == 0) ? 1u : 0u;
     for (uint64_t i = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4; i < P.N; i += stride) {    // N % 4 == 0 on the tiled path
         const uint4 v = *reinterpret_cast<const uint4 *>(sizes + i);
         if (v.x | v.y | v.z | v.w) {

@@ -55,6 +55,15 @@ struct BlkShared {
     uint32_t n_extra[kBlkThreads / 32];
     uint32_t five;                            // some block of the tile has more than 16 components (slots need a fifth bit)
 };
+// what the kSizes instantiation needs on top (sw_sweep_measure with the largest cluster): per node, bits 0-12 the number
+// of its sites -- summed into the root of its tile-local component after the last hook (a tile has 4096 sites) -- and
+// bit 15: the component owns a site on the border of the tile
+struct BlkSizesShared {
+    uint16_t size[kBlkSlots][kBlkThreads];
+    uint32_t n_tab;
+};
+constexpr uint32_t kBorderTabEntries = 256;   // per tile: <= 252 components can own one of the 252 border sites
+
 // The links that need the atomic pass are buffered per warp in node rows kBlkBufSlot .. kBlkSlots-1, which are
 // free unless some block of the tile has more than kBlkBufSlot components (then they are united unbuffered).
 constexpr int kBlkBufSlot = 14;
@@ -161,12 +170,18 @@ __device__ __forceinline__ void delta_swap(uint32_t &lo, uint32_t &hi, uint32_t 
 //              false: the whole lattice, dom is not looked at
 //   kCoherent  see ld_in
 //   Bar        the CTA-wide barrier of those kBlkThreads threads
-template <bool kSuper, bool kCoherent, class Bar>
+//   kSizes     also count the sites of every tile-local component.  A component that owns no site on the border of the
+//              tile IS a whole cluster: its size only raises row[2] (the largest cluster so far).  The others go to the
+//              tile's border table btab[tile][0..255] as (root's tile-local id | size << 12; 0 = unused entry) for the
+//              flip kernel, which adds them up per cluster (k_tile_flip_sizes); whole lattice only
+template <bool kSuper, bool kCoherent, class Bar, bool kSizes = false>
 __device__ __forceinline__ void
 tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8_t *spins, uint32_t *bonds,
                  uint32_t *labels, uint16_t *rootbits, TileBorder *border, TileEdges *edges, const uint2 *draws,
-                 const Params &P, const Dom &dom)
+                 const Params &P, const Dom &dom, BlkSizesShared *Zs = nullptr, uint32_t *btab = nullptr,
+                 unsigned long long *row = nullptr)
 {
+    static_assert(!(kSizes && kSuper), "the size counts are made for the whole lattice only");
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const uint32_t bx = tid & 7u, by = tid >> 3;
     const uint32_t L = kSuper ? dom.Lg : P.L;                  // row stride of label values (global site indices)
@@ -185,6 +200,10 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
 
     if (tid < kBlkThreads / 32) S.n_extra[tid] = 0;
     if (tid == 32) S.five = 0;
+    if (kSizes && tid == 64) Zs->n_tab = 0;
+    // kSizes: my sites on the border of the tile
+    const uint32_t bmask = !kSizes ? 0u : (by == 0u ? 0x000000FFu : 0u) | (by == 15u ? 0xFF000000u : 0u) |
+                                          (bx == 0u ? 0x01010101u : 0u) | (bx == 7u ? 0x80808080u : 0u);
 
     // -- spins: my 4 rows of 8, the row below (from the lane 8 up, or from memory), the column to the right
     uint2 s[5];
@@ -325,6 +344,7 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
                 if (k & 4) Q2 |= m;
                 if (k & 8) Q3 |= m;
                 if (k & 16) P4 |= m;
+                if (kSizes) Zs->size[k][tid] = (uint16_t)(__popc(m) | ((m & bmask) ? 0x8000u : 0u));
                 const uint32_t j = __ffs(m) - 1u;
                 S.node[k][tid] = ((idbase + ((j >> 3) << 6) + (j & 7u)) << 16) + ((uint32_t)k * 512u + my16);
             }
@@ -411,6 +431,7 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
 
     // -- every component: its root (chase, then point my node straight at it: the labels below read it from there)
     uint32_t rootm = ~todo;                                    // a site without any bond is its own cluster
+    uint32_t rootk = 0;                                        // kSizes: bit k = my node k is a root
     for (uint32_t k = 0; k < n; ++k) {
         const uint32_t me = (k << 9) + mybase;
         auto at = [win](uint32_t e) { return (e & kOffMask) | win; };
@@ -419,7 +440,40 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
         uint32_t r = r2, g = ld_node_quiet(at(r2));
         while (g != r) { r = g; g = ld_node_quiet(at(r)); }
         if (r != r1) st_node(me, r);
-        if (at(r) == me) rootm |= 1u << (((r >> 19) & 24u) | ((r >> 16) & 7u));   // my seed (y * 64 + x): bit 8 (y % 4) + x % 8
+        if (at(r) == me) {
+            rootm |= 1u << (((r >> 19) & 24u) | ((r >> 16) & 7u));   // my seed (y * 64 + x): bit 8 (y % 4) + x % 8
+            if (kSizes) rootk |= 1u << k;
+        } else if (kSizes) {                                   // my sites count for the root (two 16-bit fields per word)
+            const uint32_t idx = (at(r) - (mybase - (tid << 2))) >> 2;            // node index 128 k' + tid' of the root
+            uint32_t *const word = reinterpret_cast<uint32_t *>(&Zs->size[0][0]) + (idx >> 1);
+            const uint32_t sh = (idx & 1u) << 4, mine = Zs->size[k][tid];
+            atomicAdd(word, (mine & 0x1FFFu) << sh);
+            if (mine & 0x8000u) atomicOr(word, 0x8000u << sh);
+        }
+    }
+    if (kSizes) {
+        Bar::sync();                                           // all counts are in; pub[] is free (the table is built there)
+        uint32_t *const tab = reinterpret_cast<uint32_t *>(&S.pub[0]);
+        uint32_t whole = 0;                                    // largest component of mine that lies inside the tile
+        while (rootk) {
+            const uint32_t k = __ffs(rootk) - 1u;
+            rootk &= rootk - 1u;
+            const uint32_t f = Zs->size[k][tid], total = f & 0x1FFFu;
+            if (f & 0x8000u) tab[atomicAdd(&Zs->n_tab, 1u)] = (S.node[k][tid] >> 16) | (total << 12);   // a root holds its own entry: its seed
+            else whole = max(whole, total);
+        }
+        uint32_t lone = ~todo & bmask;                         // border sites without a bond inside the tile: components of one
+        while (lone) {
+            const uint32_t j = __ffs(lone) - 1u;
+            lone &= lone - 1u;
+            tab[atomicAdd(&Zs->n_tab, 1u)] = (idbase + ((j >> 3) << 6) + (j & 7u)) | (1u << 12);
+        }
+        whole = __reduce_max_sync(0xFFFFFFFFu, whole);
+        if (lane == 0 && whole) atomicMax(row + 2, (unsigned long long)whole);
+        Bar::sync();
+        const uint32_t n_tab = Zs->n_tab;
+#pragma unroll
+        for (uint32_t e = tid; e < kBorderTabEntries; e += kBlkThreads) btab[tile * kBorderTabEntries + e] = e < n_tab ? tab[e] : 0u;
     }
 
     // -- labels: a tile-local root keeps its own global index (the merge links it from there), every other site
@@ -501,6 +555,18 @@ k_tile_blocks(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
 {
     __shared__ BlkShared S;
     tile_blocks_body<false, false, CtaBar>(S, blockIdx.x, blockIdx.y, spins, bonds, labels, rootbits, border, edges, draws, P, Dom{});   // grid = (tiles_x, tiles_x): no division
+}
+
+// the same, and the sizes of the tile-local components (see kSizes)
+__global__ void __launch_bounds__(kBlkThreads, 9)
+k_tile_blocks_sizes(const uint8_t *__restrict__ spins, uint32_t *__restrict__ bonds,
+                    uint32_t *__restrict__ labels, uint16_t *__restrict__ rootbits,
+                    TileBorder *__restrict__ border, TileEdges *__restrict__ edges, const uint2 *__restrict__ draws, Params P,
+                    uint32_t *__restrict__ btab, unsigned long long *__restrict__ row)
+{
+    __shared__ BlkShared S;
+    __shared__ BlkSizesShared Z;
+    tile_blocks_body<false, false, CtaBar, true>(S, blockIdx.x, blockIdx.y, spins, bonds, labels, rootbits, border, edges, draws, P, Dom{}, &Z, btab, row);
 }
 
 // the same for one sub-lattice of the super-lattice (sw_super.cu); grid = (W / 64, H / 64)

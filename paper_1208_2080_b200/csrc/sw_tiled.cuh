@@ -234,12 +234,6 @@ struct FlipShared {
     uint16_t list[NT / 32][kRows * kTile];                       // per warp: the tile-local roots of its rows
 };
 
-// what the kSizes instantiation of the flip body needs on top of FlipShared
-struct FlipSizesShared {
-    uint32_t cnt[kTileSites];                                    // per tile-local root: how many sites of the tile carry it
-    uint32_t touch[kTileSites / 32];                             // bit id: the tile-local root `id` owns a site on the tile border
-};
-
 // The body of the flip kernel for tile (tx, ty), run by NT threads.
 // kLabels: write the canonical labels back (eager mode, or the on-demand flatten of lazy mode);
 // kSpins: draw and write the new spins; kCount: leave the number of canonical roots per warp in tile_clusters[]
@@ -247,16 +241,17 @@ struct FlipSizesShared {
 // kSuper: one sub-lattice of the super-lattice: label values global, addresses local; a chase ends at a root OR at the
 // first link that leaves the piece (after the resolve pass of sw_super.cu such a link points at the canonical root).
 // pk_t / pk_n: philox_sweep constants of this sweep and the next (Params::pk_t / pk_n, or made on the device).
-// kSizes (sw_sweep_measure with the largest cluster): the cluster sizes are counted here as well, per tile-local root in
-// shared memory; a root that owns no site on the tile border and was never hooked IS a whole cluster (its count only
-// feeds the maximum in row[2]), every other root adds its count to sizes[canonical root] -- one global atomic per
-// tile-local component that crosses a tile border instead of one per run of sites in a separate pass over labels[].
+// kSizes (sw_sweep_measure with the largest cluster): the tile kernel listed the tile-local components that own a site on
+// the border of the tile in btab[tile][] (root's tile-local id | size << 12, k_tile_blocks_sizes; the others are whole
+// clusters and were dealt with there); each adds its size to sizes[canonical root] -- one global atomic per such
+// component, nothing per site -- so that afterwards sizes[] (all zero before) holds the sizes of the clusters that
+// cross a tile border at their canonical roots.
 template <bool kLabels, bool kSpins, bool kCount, bool kStats, bool kSuper, int NT, class Bar, bool kSizes = false>
 __device__ __forceinline__ void
 tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t *labels, const uint16_t *rootbits, uint8_t *spins,
                const Params &P, const uint32_t (&pk_t)[3], const uint32_t (&pk_n)[3], const Dom &dom,
-               uint32_t *tile_clusters, uint2 *next_draws, PassCounters *counters,
-               FlipSizesShared *Z = nullptr, uint32_t *sizes = nullptr, unsigned long long *row = nullptr)
+               uint32_t *tile_clusters, uint2 *next_draws, PassCounters *counters, uint32_t *sizes = nullptr,
+               const uint32_t *btab = nullptr)
 {
     constexpr int kAcc = FlipShared<NT>::kAcc, kRows = FlipShared<NT>::kRows;
     const uint32_t tid = threadIdx.x;
@@ -278,10 +273,10 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
     //    register, so the 16 sites of a thread cost 8 registers across the chases instead of 16.
     uint32_t work = 0;                                         // bit 4k + j: my site j of access k is a tile-local root
     uint32_t rq[kAcc];
+    uint32_t tab = 0;                                          // kSizes: my entry of the tile's border table
     if (kSizes) {
-        for (uint32_t k = tid; k < kTileSites; k += NT) Z->cnt[k] = 0;
-        if (tid < kTileSites / 32) Z->touch[tid] = 0;
-        Bar::sync();
+        static_assert(!kSizes || NT == 256, "one border-table entry per thread");
+        tab = __ldcg(btab + tile * 256u + tid);
     }
     // The labels go straight to shared memory (cp.async, L2 only: 16 bytes per thread and access, no registers held
     // while they are in flight): a root's entry is where its chase starts (and is replaced by the canonical root
@@ -302,23 +297,7 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
 #pragma unroll
     for (int k = 0; k < kAcc; ++k) work |= ((rq[k] >> (x4 & 12u)) & 15u) << (4 * k);
     asm volatile("cp.async.wait_all;" ::: "memory");
-    if (kSizes) {                                              // border sites of the tile mark their root
-#pragma unroll
-        for (int k = 0; k < kAcc; ++k) {
-            const uint32_t id0 = ((yk0 + 2 * k) << 6) + x4, rb = (work >> (4 * k)) & 15u;
-            const uint4 l = *reinterpret_cast<const uint4 *>(&S.root[id0]);
-            const uint32_t lab[4] = {l.x, l.y, l.z, l.w};
-            const uint32_t y = yk0 + 2 * k;
-            const bool row_edge = y == 0 || y + 1 == kTile;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const uint32_t id = ((rb >> j) & 1u) ? id0 + j : lab[j];
-                if (row_edge || x4 + j == 0 || x4 + j + 1 == kTile) atomicOr(&Z->touch[id >> 5], 1u << (id & 31u));
-            }
-        }
-    }
 
-    uint32_t n_warp_roots = 0;
     {
         // each warp lists the tile-local roots of its rows (prefix sum over the lanes, no atomics) ...
         const uint32_t n = __popc(work);
@@ -329,7 +308,6 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
             if (lane >= (uint32_t)o) incl += up;
         }
         const uint32_t n_warp = __shfl_sync(0xFFFFFFFFu, incl, 31);
-        n_warp_roots = n_warp;
         uint32_t pos = incl - n, w = work;
         const uint32_t idb = (yk0 << 6) + x4;
         while (w) {
@@ -364,6 +342,7 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
         }
     }
     Bar::sync();
+    if (kSizes && (tab >> 12)) atomicAdd(sizes + S.root[tab & 0xFFFu], tab >> 12);   // (the root's entry holds its canonical root now)
 
     // -- phase C: every site looks up (canonical root, new state) of its tile-local root
     uint32_t canon = 0;                                        // clusters whose smallest site is one of mine (for sw_measure)
@@ -385,19 +364,6 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
             if (kCount) canon += (lab[j] == i0 + j);           // a canonical root is its own label
             if (kSpins) st |= (uint32_t)S.state[id] << (8 * j);
         }
-        if (kSizes) {
-            // my 4 sites count for their tile-local roots, runs of equal ids together; a root does not count itself (it is
-            // added when the counts are read), so singletons -- a quarter of the sites at q = 10 -- cost no atomic at all
-            const uint32_t rb = (work >> (4 * k)) & 15u;
-            uint32_t cur = qid[0], len = (rb & 1u) ^ 1u;
-#pragma unroll
-            for (int j = 1; j < 4; ++j) {
-                const uint32_t w = ((rb >> j) & 1u) ^ 1u;
-                if (qid[j] == cur) len += w;
-                else { if (len) atomicAdd(&Z->cnt[cur], len); cur = qid[j]; len = w; }
-            }
-            if (len) atomicAdd(&Z->cnt[cur], len);
-        }
         if (kSpins) *reinterpret_cast<uint32_t *>(spins + o) = st;
         if (kLabels)
             *reinterpret_cast<uint4 *>(labels + o) = make_uint4(lab[0], lab[1], lab[2], lab[3]);
@@ -405,18 +371,6 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
     if (kCount) {
         canon = __reduce_add_sync(0xFFFFFFFFu, canon);
         if (lane == 0) tile_clusters[tile * (NT / 32) + warp] = canon;
-    }
-    if (kSizes) {
-        Bar::sync();                                           // all counts of the tile are in
-        uint32_t whole = 0;                                    // largest cluster that lies entirely inside this tile
-        for (uint32_t k = lane; k < n_warp_roots; k += 32) {
-            const uint32_t id = S.list[warp][k], n = Z->cnt[id] + 1u, g = S.root[id];
-            const uint32_t self = origin + (id >> 6) * L + (id & 63u);
-            if (g != self || ((Z->touch[id >> 5] >> (id & 31u)) & 1u)) atomicAdd(sizes + (kSuper ? DomAddr(dom)(g) : g), n);
-            else whole = max(whole, n);
-        }
-        whole = __reduce_max_sync(0xFFFFFFFFu, whole);
-        if (lane == 0 && whole) atomicMax(row + 2, (unsigned long long)whole);
     }
 }
 
@@ -434,15 +388,14 @@ k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__
 }
 
 // the flip of a sweep whose cluster sizes are wanted (sw_sweep_measure with SW_OBS_LARGEST): eager labels, spins, cluster
-// count, and the sizes (see tile_flip_body, kSizes); sizes[] must be all zero before, row[2] is only raised
-__global__ void __launch_bounds__(kFlipThreads, 4)
+// count, and the sizes (see tile_flip_body, kSizes; the tile kernel of this sweep was k_tile_blocks_sizes)
+__global__ void __launch_bounds__(kFlipThreads, SW_FLIP_CTAS)
 k_tile_flip_sizes(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__restrict__ spins, Params P,
-                  uint32_t *__restrict__ tile_clusters, uint2 *__restrict__ next_draws, uint32_t *sizes, unsigned long long *row)
+                  uint32_t *__restrict__ tile_clusters, uint2 *__restrict__ next_draws, uint32_t *sizes, const uint32_t *__restrict__ btab)
 {
     __shared__ FlipShared<kFlipThreads> S;
-    __shared__ FlipSizesShared Z;
     tile_flip_body<true, true, true, false, false, kFlipThreads, MergeBar, true>(
-        S, blockIdx.x, blockIdx.y, labels, rootbits, spins, P, P.pk_t, P.pk_n, Dom{}, tile_clusters, next_draws, nullptr, &Z, sizes, row);
+        S, blockIdx.x, blockIdx.y, labels, rootbits, spins, P, P.pk_t, P.pk_n, Dom{}, tile_clusters, next_draws, nullptr, sizes, btab);
 }
 
 // one sub-lattice of the super-lattice; grid = (W / 64, H / 64).  `spins` is read by the neighbours' tile kernels of the
