@@ -52,9 +52,10 @@ def test_workspace_plan_no_device_needed(libsw):
         n = binding.workspace_bytes(L, q)
         N = L * L
         assert n >= N + N // 4 + 4 * N                       # spins + bond bits + labels
-        # + tile-root bitmap, border / edge records, draw bits, cluster counts, and the context-owned scratch:
-        # the row ring of sw_sweep_measure (<= 256 KiB), the staging buffer of sw_get_bonds (min(N, 32 MiB)), pass counters
-        assert n <= 7.0 * N + 8192 + (256 << 10)
+        # + tile-root bitmap, border / edge records, border table of the cluster-size count (0.25 B/site), draw bits, cluster
+        # counts, and the context-owned scratch: the row ring of sw_sweep_measure (<= 256 KiB), the staging buffer of
+        # sw_get_bonds (min(N, 32 MiB)), pass counters
+        assert n <= 7.25 * N + 8192 + (256 << 10)
         assert binding.workspace_bytes(L, q, binding.FLAG_WS_CLUSTER_SIZES) >= n + 4 * N      # the optional cluster-size scratch
     # headline size: 2^32 sites must fit one B200 with room to spare (180 GB)
     n = binding.workspace_bytes(65536, 2)
