@@ -482,8 +482,9 @@ def test_packed_state_needs_enough_bits_and_a_multiple_of_16_sites():
                                          (384, 2, wl.k_critical(2), "ordered"), (320, 2, math.inf, "ordered"), (320, 4, 0.0, "random"),
                                          (192, 2, wl.k_critical(2), "random")])
 def test_series_with_cluster_sizes_counted_in_the_flip_kernel(L, q, K, start):
-    # sw_sweep_measure with the largest cluster on the three-kernel path: the sizes are counted by k_tile_flip_sizes
-    # (clusters inside one tile never touch global memory); every row must equal the oracle's, whatever is asked before and after
+    # sw_sweep_measure with the largest cluster on the three-kernel path: the sizes are counted along the union-find of
+    # k_tile_blocks_sizes (clusters inside one tile never touch global memory, the others go through the tile's border
+    # table to k_tile_flip_sizes); every row must equal the oracle's, whatever is asked before and after
     flags = sw.FLAG_NO_CLUSTER_PATH
     gpu, cpu = SwendsenWang(L, q, K, 12, flags=flags), Oracle(L, q, K, 12)
     gpu.init(start); cpu.init(start)
@@ -504,6 +505,14 @@ def test_cluster_sizes_in_the_flip_kernel_on_adversarial_lattices():
         gpu, cpu = SwendsenWang(L, 3, math.inf, 1), Oracle(L, 3, math.inf, 1)
         gpu.set_state(spins, 2); cpu.set_state(spins, 2)
         assert np.array_equal(gpu.sweep_measure(2), cpu.sweep_measure(2)), name
+    # dominoes that straddle the tile borders: both halves are border sites without a bond inside their tile (components of
+    # one in the border table), and the canonical root of the pair is such a site
+    for vertical in (False, True):
+        spins = wl.spins_dominoes(L, 1, 1, vertical)
+        gpu, cpu = SwendsenWang(L, 251, math.inf, 1), Oracle(L, 251, math.inf, 1)
+        gpu.set_state(spins, 5); cpu.set_state(spins, 5)
+        want = cpu.sweep_measure(1)
+        assert np.array_equal(gpu.sweep_measure(1), want) and want[0, 2] >= 2, f"dominoes vertical={vertical}"
     big = SwendsenWang(1024, 2, wl.k_critical(2), 3, flags=sw.FLAG_WS_CLUSTER_SIZES)
     ref = Oracle(1024, 2, wl.k_critical(2), 3)
     big.init("ordered"); ref.init("ordered")
