@@ -40,10 +40,9 @@ constexpr uint32_t kOffMask = 0xFFFFu;        // the address half of a node entr
 // (the seed = smallest site of the component, as a tile-local id y * 64 + x; static shared memory lies in the first
 // 64 KB of the CTA's window, so 16 bits hold the address and a hop is one logic instruction + one load; the upper
 // bits `win` of a shared address are the same for the whole CTA: zero, or the rank of the CTA in its cluster); a
-// root holds its own.  Entries are unique per
-// node and ordered like the seeds, so hooking the larger root under the smaller is one native 32-bit atomicMin, the
-// root of a tile-local component is its smallest site, and the upper half of a root's entry IS the label
-// of the component's other sites.
+// root holds its own.  Entries are unique per node and ordered like the seeds, so hooking the larger root under the
+// smaller is one native 32-bit atomicMin, the root of a tile-local component is its smallest site, and
+// the upper half of a root's entry IS the label of the component's other sites.
 struct BlkShared {
     uint32_t node[kBlkSlots][kBlkThreads];    // flood fill: component masks; then the entries (see above); rows >= kBlkBufSlot double as link buffer
     uint4 pub[kBlkThreads];                   // what the blocks below / to the right need to know about my components:
