@@ -517,3 +517,22 @@ def test_cluster_sizes_in_the_flip_kernel_on_adversarial_lattices():
     ref = Oracle(1024, 2, wl.k_critical(2), 3)
     big.init("ordered"); ref.init("ordered")
     assert np.array_equal(big.sweep_measure(5, sw.OBS_CLUSTERS | sw.OBS_LARGEST)[:, 1:3], ref.sweep_measure(5)[:, 1:3])
+
+
+@pytest.mark.parametrize("L,q,K,start,n", [(2048, 2, wl.k_critical(2), "ordered", 120), (2048, 10, wl.k_critical(10) * 1.005, "random", 120),
+                                           (1024, 3, 0.3, "random", 60), (1024, 2, 2.0, "random", 60)])
+def test_repeated_runs_are_bitwise_identical(L, q, K, start, n):
+    # compute-sanitizer's racecheck is closed on this pool; what a race in the shared-memory union-find, the cp.async staging
+    # or the global merge would do is make long runs differ from one another: three independent contexts, the same seed,
+    # sizes counted every sweep, and every row, spin and label must agree (the comparison with the oracle is made elsewhere)
+    res = []
+    for _ in range(3):
+        g = SwendsenWang(L, q, K, 7)
+        g.init(start)
+        rows = g.sweep_measure(n)
+        g.sweep(17)
+        res.append((g.get_spins(), g.get_labels(), rows, g.measure()))
+        g.close()
+    for r in res[1:]:
+        assert np.array_equal(res[0][0], r[0]) and np.array_equal(res[0][1], r[1])
+        assert np.array_equal(res[0][2], r[2]) and res[0][3] == r[3]
