@@ -269,8 +269,8 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
     // -- phase A: everything this tile needs from HBM is requested at once: my labels and root flags.
     //    A tile-local root's own entry is its link into the global forest (itself if the merge never hooked
     //    it), so the first step of every chase comes out of this coalesced load instead of a scattered one.
-    //    What a site needs afterwards is the tile-local id of its root (12 bits; its own id if it is a root): two per
-    //    register, so the 16 sites of a thread cost 8 registers across the chases instead of 16.
+    //    What a site needs afterwards is the tile-local id of its root (12 bits; its own id if it is a root): it stays
+    //    in shared memory until phase C.
     uint32_t work = 0;                                         // bit 4k + j: my site j of access k is a tile-local root
     uint32_t rq[kAcc];
     uint32_t tab = 0;                                          // kSizes: my entry of the tile's border table
