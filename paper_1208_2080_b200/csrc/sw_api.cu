@@ -288,8 +288,10 @@ int sweep_once(sw_ctx *c, bool count_clusters, unsigned long long *sizes_row = n
         { Timed tm(c, SLOT_TILE);
           sw::k_tile_blocks<<<tgrid, sw::kBlkThreads, 0, c->stream>>>(c->d_spins, c->d_bonds, c->d_labels, c->d_rootbits, c->d_border, c->d_edges, c->d_draws, P); }
         { Timed tm(c, SLOT_MERGE);
-          auto merge = c->count_passes ? sw::k_tile_merge<true> : sw::k_tile_merge<false>;
-          merge<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_edges, P, tiles, c->d_counters); }
+          const unsigned per = (unsigned)sw::merge_tiles_per_cta(tiles);
+          auto merge = per == 2 ? (c->count_passes ? sw::k_tile_merge<true, 2> : sw::k_tile_merge<false, 2>)
+                                : (c->count_passes ? sw::k_tile_merge<true, 4> : sw::k_tile_merge<false, 4>);
+          merge<<<(tiles + per - 1) / per, sw::kMergeThreads, 0, c->stream>>>(c->d_labels, c->d_border, c->d_edges, P, tiles, c->d_counters); }
         if (with_sizes) {
             Timed tm(c, SLOT_FLIP);
             sw::k_tile_flip_sizes<<<tgrid, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, c->d_draws, c->d_sizes, c->d_btab);

@@ -406,7 +406,9 @@ int super_phase(sw_super *s, int phase, bool count_clusters)
         if (phase == 0) {
             if (s->draws_t != s->t) { sw::k_draws_super<<<tgrid, 256, 0, p.stream>>>(p.draws, P, p.dom); s->launches += 1; }
             sw::k_tile_blocks_super<<<tgrid, sw::kBlkThreads, 0, p.stream>>>(p.spins, p.bonds, p.labels, p.rootbits, p.border, p.edges, p.draws, P, p.dom);
-            sw::k_tile_merge_super<<<(tiles + sw::kMergeTiles - 1) / sw::kMergeTiles, sw::kMergeThreads, 0, p.stream>>>(p.labels, p.border, p.edges, P, p.dom, tiles);
+            const unsigned per = (unsigned)sw::merge_tiles_per_cta(tiles);
+            auto merge = per == 2 ? sw::k_tile_merge_super<2> : sw::k_tile_merge_super<4>;
+            merge<<<(tiles + per - 1) / per, sw::kMergeThreads, 0, p.stream>>>(p.labels, p.border, p.edges, P, p.dom, tiles);
             SS_CUDA(s, cudaEventRecord(p.ev_stage1, p.stream));
             s->launches += 2;
         } else if (phase == 1) {

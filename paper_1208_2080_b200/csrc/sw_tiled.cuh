@@ -102,20 +102,23 @@ k_draws_super(uint2 *__restrict__ draws, Params P, Dom dom)
 // One thread per border site (64 on the right column, 64 on the bottom row of a tile).  Only about a
 // third of them carry a link worth uniting (active bond, not a repeat of its neighbour's link), and a
 // unite is a chain of dependent L2 / HBM round trips, so the kernel is latency-bound: a CTA therefore
-// gathers the links of kMergeTiles tiles into a dense list first (coalesced loads, all independent)
-// and then unites them with every lane busy.
+// gathers the links of kTiles tiles into a dense list first (coalesced loads, all independent)
+// and then unites them with every lane busy.  kTiles = 4 for the largest lattices; up to L = 16384 (65536 tiles) two
+// tiles per CTA are faster -- more, shorter CTAs: 18.6 instead of 25.3 us at L = 4096 (config 2, where the merge is a
+// fifth of the sweep), 35.9 instead of 38.3 us at L = 8192; at L = 65536 four win by 2 % (merge_tiles_per_cta).
 
-constexpr int kMergeTiles = 4;
+constexpr int kMergeTiles = 4;                       // the most a CTA takes (MergeShared is sized for it)
+__host__ __device__ constexpr int merge_tiles_per_cta(unsigned n_tiles) { return n_tiles <= 65536u ? 2 : 4; }
 
 struct MergeShared {
     uint2 link[kMergeTiles * kMergeThreads];
     uint32_t n;
 };
 
-// The links of tiles [tile_begin, tile_end) (at most kMergeTiles of them), by kMergeThreads threads.
+// The links of tiles [tile_begin, tile_end) (at most kTiles of them), by kMergeThreads threads.
 //   kSuper: borders that leave the piece are NOT united here (the inter-domain merge of sw_super.cu does that,
 //   PAPER.md:66-68); label values are global, addresses local (DomAddr).
-template <bool kStats, bool kSuper, bool kCoherent, class Bar>
+template <bool kStats, bool kSuper, bool kCoherent, class Bar, int kTiles = kMergeTiles>
 __device__ __forceinline__ void
 tile_merge_body(MergeShared &S, uint32_t *labels, const TileBorder *border, const TileEdges *edges, const Params &P, const Dom &dom,
                 const uint32_t tile_begin, const uint32_t tile_end, PassCounters *counters)
@@ -125,10 +128,11 @@ tile_merge_body(MergeShared &S, uint32_t *labels, const TileBorder *border, cons
     if (b == 0) S.n = 0;
     Bar::sync();
 
-    uint32_t lu[kMergeTiles], lv[kMergeTiles];
-    bool on[kMergeTiles];
+    static_assert(kTiles <= kMergeTiles, "MergeShared holds the links of kMergeTiles tiles");
+    uint32_t lu[kTiles], lv[kTiles];
+    bool on[kTiles];
 #pragma unroll
-    for (int i = 0; i < kMergeTiles; ++i) {
+    for (int i = 0; i < kTiles; ++i) {
         const uint32_t tile = tile_begin + i;
         on[i] = false; lu[i] = 0; lv[i] = 0;
         if (tile < tile_end) {
@@ -158,7 +162,7 @@ tile_merge_body(MergeShared &S, uint32_t *labels, const TileBorder *border, cons
         }
     }
 #pragma unroll
-    for (int i = 0; i < kMergeTiles; ++i) {
+    for (int i = 0; i < kTiles; ++i) {
         // the previous border bond joins the same two tile-local components: nothing new to learn
         const uint32_t plu = __shfl_up_sync(0xFFFFFFFFu, lu[i], 1), plv = __shfl_up_sync(0xFFFFFFFFu, lv[i], 1);
         const bool pon = __shfl_up_sync(0xFFFFFFFFu, (uint32_t)on[i], 1) != 0;
@@ -194,21 +198,22 @@ struct MergeBar {
     static __device__ __forceinline__ void sync() { __syncthreads(); }
 };
 
-template <bool kStats>
+template <bool kStats, int kTiles>
 __global__ void __launch_bounds__(kMergeThreads)
 k_tile_merge(uint32_t *labels, const TileBorder *__restrict__ border, const TileEdges *__restrict__ edges,
              Params P, uint32_t n_tiles, PassCounters *__restrict__ counters)
 {
     __shared__ MergeShared S;
-    tile_merge_body<kStats, false, false, MergeBar>(S, labels, border, edges, P, Dom{}, blockIdx.x * kMergeTiles, n_tiles, counters);
+    tile_merge_body<kStats, false, false, MergeBar, kTiles>(S, labels, border, edges, P, Dom{}, blockIdx.x * kTiles, n_tiles, counters);
 }
 
+template <int kTiles>
 __global__ void __launch_bounds__(kMergeThreads)
 k_tile_merge_super(uint32_t *labels, const TileBorder *__restrict__ border, const TileEdges *__restrict__ edges,
                    Params P, Dom dom, uint32_t n_tiles)
 {
     __shared__ MergeShared S;
-    tile_merge_body<false, true, false, MergeBar>(S, labels, border, edges, P, dom, blockIdx.x * kMergeTiles, n_tiles, nullptr);
+    tile_merge_body<false, true, false, MergeBar, kTiles>(S, labels, border, edges, P, dom, blockIdx.x * kTiles, n_tiles, nullptr);
 }
 
 // ---- kernel 3: flatten to the canonical root + flip --------------------------------------------
