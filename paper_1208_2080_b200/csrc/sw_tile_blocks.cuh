@@ -248,6 +248,15 @@ tile_blocks_body(BlkShared &S, const uint32_t tx, const uint32_t ty, const uint8
                 R |= (pack4(~(a0 ^ n0)) | (pack4(~(a1 ^ n1)) << 4)) << (8 * r);
                 D |= (pack4(~(a0 ^ s[r + 1].x)) | (pack4(~(a1 ^ s[r + 1].y)) << 4)) << (8 * r);
             }
+        } else if (P.q <= 4u) {                                // states are two bits: equal iff the XOR has neither (bit 0 of the NOR)
+            auto eq2 = [](uint32_t a, uint32_t b) { const uint32_t d = a ^ b; return ~(d | (d >> 1)); };
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const uint32_t a0 = s[r].x, a1 = s[r].y;
+                const uint32_t n0 = __funnelshift_r(a0, a1, 8), n1 = __funnelshift_r(a1, nx >> (8 * r), 8);
+                R |= (pack4(eq2(a0, n0)) | (pack4(eq2(a1, n1)) << 4)) << (8 * r);
+                D |= (pack4(eq2(a0, s[r + 1].x)) | (pack4(eq2(a1, s[r + 1].y)) << 4)) << (8 * r);
+            }
         } else {
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
