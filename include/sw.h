@@ -278,6 +278,44 @@ int  sw_xy_get_reflection(sw_xy *c, double r[2]);  /* the direction r of the las
 int  sw_xy_get_time(sw_xy *c, uint64_t *t);
 const char *sw_xy_last_error(const sw_xy *c);
 
+/* --- cluster statistics without any device allocation ----------------------------------------------------------------
+ * Who this is for.  sw_measure(largest_cluster) and sw_measure_clusters keep one uint32 counter per site, 4*L*L bytes,
+ * which the library cudaMalloc's the first time it is needed (or takes from the workspace, SW_FLAG_WS_CLUSTER_SIZES).
+ * Some programs cannot let a library do that: every byte of the GPU already belongs to the program's own memory pool, so
+ * a cudaMalloc made behind its back fails or shrinks what the pool counted on; or the call sits inside a sweep loop that
+ * cannot stop for the device-wide synchronisation an allocation brings with it; or the memory budget of the job was
+ * fixed when the library was loaded and must not move afterwards.  sw_cluster_stats_static is the counting pass of
+ * PAPER.md:42 / BASELINE.json config 4 (sites per cluster, keyed by the cluster's smallest site) for those callers: its
+ * counters live in an array that is compiled into libsw.so (static __device__, SW_STATIC_MAX_SITES uint32 = 4 MiB on
+ * every GPU that loads the library, held until the process exits), and the call itself allocates and frees nothing, on
+ * the device or on the host.
+ *
+ *   dev_labels  DEVICE uint32[n_sites], on the current device: canonical labels, labels[i] = smallest site of i's
+ *               cluster (what sw_get_labels returns), owned by the caller, only read
+ *   n_sites     0 .. SW_STATIC_MAX_SITES (L <= 1024); anything larger -> SW_ERR_INVALID_ARG, nothing is launched and
+ *               sw_static_last_error() says so: larger lattices have to go through sw_measure_clusters
+ *   dev_out     DEVICE uint64[4], on the current device, owned by the caller, overwritten:
+ *               [0] number of clusters, [1] size of the largest, [2] sum over clusters of size^2 (< 2^64 at this size),
+ *               [3] number of sites whose label is not a canonical root of this lattice (>= n_sites, or
+ *               labels[label] != label); such sites are left out of [0..2], so [3] != 0 means "bad input"
+ *   cuda_stream cudaStream_t of the current device (NULL = the legacy default stream); three small kernels are enqueued
+ *               on it and the call returns without waiting.  Read dev_out after synchronising that stream.
+ *
+ * Shared scratch.  There is ONE array per GPU and every call on that GPU uses it.  A call clears the part it needs
+ * before counting, so nothing survives from the call before (whose counts stay in the array until then); but two calls
+ * whose kernels can run at the same time on one GPU -- different streams, different host threads, different contexts
+ * of this process -- count into the same words and both results are garbage.  Keep calls on one GPU in one stream, or
+ * order them with events.
+ * First call on a device.  The array's device address is looked up once per device (cudaGetSymbolAddress, with that
+ * device current) by the first call made there, which may also make the runtime load the library's kernels.  Make that
+ * first call during start-up, before any stream capture is begun.
+ * Errors.  SW_ERR_INVALID_ARG (NULL, n_sites too large, a pointer that is not memory of the current device) or
+ * SW_ERR_CUDA; sw_static_last_error() returns the reason of the calling thread's last failure ("" after a success).  */
+#define SW_STATIC_MAX_SITES (1u << 20)
+int sw_cluster_stats_static(const uint32_t *dev_labels, uint64_t n_sites, uint64_t *dev_out, void *cuda_stream);
+uint64_t sw_static_max_sites(void);            /* SW_STATIC_MAX_SITES, for callers that bind at run time */
+const char *sw_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -36,6 +36,7 @@ SYMBOLS = [
     "sw_create_super_rank", "sw_super_ipc_export", "sw_super_ipc_import", "sw_super_phase", "sw_super_measure_phase",
     "sw_xy_create", "sw_xy_destroy", "sw_xy_init", "sw_xy_set_state", "sw_xy_sweep", "sw_xy_measure", "sw_xy_get_spins",
     "sw_xy_get_labels", "sw_xy_get_bonds", "sw_xy_get_reflection", "sw_xy_get_time", "sw_xy_last_error",
+    "sw_cluster_stats_static", "sw_static_max_sites", "sw_static_last_error",
 ]
 
 
@@ -128,6 +129,9 @@ def lib():
     l.sw_xy_get_reflection.argtypes = [vp, dp]
     l.sw_xy_get_time.argtypes = [vp, u64p]
     l.sw_xy_last_error.argtypes = [vp]; l.sw_xy_last_error.restype = C.c_char_p
+    l.sw_cluster_stats_static.argtypes = [vp, C.c_uint64, vp, vp]
+    l.sw_static_max_sites.argtypes = []; l.sw_static_max_sites.restype = C.c_uint64
+    l.sw_static_last_error.argtypes = []; l.sw_static_last_error.restype = C.c_char_p
     for name in SYMBOLS:
         getattr(l, name)                         # AttributeError here = the library is stale
     _lib = l
@@ -136,6 +140,22 @@ def lib():
 
 def workspace_bytes(L, q, flags=FLAG_DEFAULT):
     return int(lib().sw_workspace_bytes(L, q, flags))
+
+
+def static_max_sites():
+    return int(lib().sw_static_max_sites())
+
+
+def cluster_stats_static(dev_labels_ptr, n_sites, dev_out_ptr, cuda_stream=0):
+    """sw_cluster_stats_static: cluster count, largest cluster and sum of squared sizes of `n_sites` canonical labels,
+    for callers that must not allocate on the device (the counters are a fixed array inside libsw.so; at most
+    static_max_sites() sites).  All three pointers are raw DEVICE addresses / a cudaStream_t as integers; the result
+    (uint64[4] at dev_out_ptr) is ready once the stream has been synchronised.  Calls on one GPU share the counters:
+    keep them on one stream."""
+    rc = lib().sw_cluster_stats_static(C.c_void_p(dev_labels_ptr), int(n_sites), C.c_void_p(dev_out_ptr), C.c_void_p(cuda_stream))
+    if rc != OK:
+        msg = lib().sw_static_last_error()
+        raise SwError(rc, "sw_cluster_stats_static", msg.decode() if msg else "")
 
 
 class SwendsenWang:
