@@ -83,6 +83,7 @@ struct sw_ctx {
     bool tiled = false, lazy = false, label_equiv = false;
     bool cluster = false;                 // small lattice: all sweeps of a call in ONE launch of k_cluster_sweeps (sw_cluster.cuh)
     uint32_t counts_per_tile = sw::kFlipThreads / 32;   // entries per tile the last flip left in d_tile_clusters
+    uint64_t counts_t = ~0ull;            // == t: d_tile_clusters holds the root counts of the last sweep (a flip with kCount ran)
     uint64_t le_rounds_last = 0, le_rounds_total = 0;
     bool have_spins = false, have_labels = false, labels_flat = false;
     bool owns_ws = false, owns_stream = false;
@@ -149,15 +150,7 @@ int cuda_fail(sw_ctx *c, cudaError_t e, const char *what)
         if (e_ != cudaSuccess) return cuda_fail((c), e_, #call);    \
     } while (0)
 
-// north_star: T = floor(p * 2^32), p = 1 - exp(-K), computed once on the host (R10)
-bool host_threshold(double K, uint64_t *T)
-{
-    if (std::isnan(K) || K < 0.0) return false;
-    if (std::isinf(K)) { *T = 1ull << 32; return true; }
-    const double scaled = std::floor(std::ldexp(-std::expm1(-K), 32));
-    *T = scaled <= 0.0 ? 0ull : (scaled >= 4294967296.0 ? (1ull << 32) : (uint64_t)scaled);
-    return true;
-}
+using swh::host_threshold;   // T = floor(p * 2^32), p = 1 - exp(-K), computed once on the host (sw_host.h; R10)
 
 Params make_params(const sw_ctx *c, uint64_t t)
 {
@@ -224,6 +217,7 @@ int sweep_cluster(sw_ctx *c, uint64_t n, uint32_t what, unsigned long long *d_ro
     c->draws_t = c->t;
     c->have_labels = true; c->labels_flat = true;
     c->counts_per_tile = sw::kClusterThreads / 32;
+    c->counts_t = c->t;                  // the cluster kernel counts the roots of every sweep
     return SW_OK;
 }
 
@@ -304,7 +298,10 @@ int sweep_once(sw_ctx *c, bool count_clusters, unsigned long long *sizes_row = n
           flip<<<tgrid, sw::kFlipThreads, 0, c->stream>>>(c->d_labels, c->d_rootbits, c->d_spins, P, c->d_tile_clusters, c->d_draws, c->d_counters); }
         c->draws_t = c->t + 1;           // the flip kernel made the draws of the next sweep on the side
         c->labels_flat = !c->lazy;
-        c->counts_per_tile = sw::kFlipThreads / 32;
+        if (with_sizes || count_clusters || c->count_passes) {     // the flip instantiations with kCount
+            c->counts_per_tile = sw::kFlipThreads / 32;
+            c->counts_t = c->t + 1;
+        }
     } else if (c->label_equiv) {
         // the loop of scanning and analysis kernels "is iterated up to the point when the information of
         // the labeling needs no more process of scanning function"; as in the paper the host looks at a flag every round
@@ -373,7 +370,12 @@ int enqueue_observe(sw_ctx *c, unsigned long long *row, bool want_e, bool want_m
     if (!row_is_zero) SW_CUDA(c, cudaMemsetAsync(row, 0, (3 + (size_t)c->q) * 8, c->stream));
     const bool cl = c->have_labels;
     uint32_t want = (want_e ? 1u : 0u) | (want_m ? 2u : 0u) | ((cl && (want_nc || want_big)) ? 4u : 0u);
-    if ((want & 4u) && c->tiled) {      // the flip kernel of the last sweep left one count per tile: no pass over labels[]
+    if ((want & 4u) && c->tiled && c->counts_t != c->t) {
+        // the last sweep ran without the count (sw_sweep_measure_ex without SW_OBS_CLUSTERS / SW_OBS_LARGEST): d_tile_clusters is
+        // stale or was never written; count the roots (labels[i] == i) in the observe pass below, on flat labels
+        const int rc = ensure_flat(c);
+        if (rc != SW_OK) return rc;
+    } else if ((want & 4u) && c->tiled) {      // the flip kernel of the last sweep left one count per tile: no pass over labels[]
         want &= ~4u;
         c->launches += 1;
         const unsigned tiles = (unsigned)(c->N / sw::kTileSites) * c->counts_per_tile;   // one count per warp of the last flip
@@ -531,7 +533,7 @@ int sw_init(sw_ctx *c, int mode)
         sw::k_init_random<<<grid_for(c, c->N, 256), 256, 0, c->stream>>>(c->d_spins, P);
         SW_CUDA(c, cudaGetLastError());
     } else return fail(c, SW_ERR_INVALID_ARG, "sw_init: unknown mode");
-    c->t = 0; c->have_spins = true; c->have_labels = false; c->labels_flat = false; c->sizes_t = ~0ull;
+    c->t = 0; c->have_spins = true; c->have_labels = false; c->labels_flat = false; c->sizes_t = ~0ull; c->counts_t = ~0ull;
     return SW_OK;
 }
 
@@ -547,7 +549,7 @@ int sw_set_state(sw_ctx *c, const uint8_t *src, uint64_t t)
     uint32_t bad = 0;
     SW_CUDA(c, cudaMemcpyAsync(&bad, c->d_flag, 4, cudaMemcpyDeviceToHost, c->stream));
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
-    c->have_labels = false; c->labels_flat = false; c->sizes_t = ~0ull;
+    c->have_labels = false; c->labels_flat = false; c->sizes_t = ~0ull; c->counts_t = ~0ull;
     if (bad) { c->have_spins = false; return fail(c, SW_ERR_INVALID_ARG, "sw_set_state: spin value >= q"); }
     c->t = t; c->have_spins = true;
     return SW_OK;
@@ -573,7 +575,7 @@ int sw_set_state_packed(sw_ctx *c, const void *src, uint32_t bits, uint64_t t)
     uint32_t bad = 0;
     SW_CUDA(c, cudaMemcpyAsync(&bad, c->d_flag, 4, cudaMemcpyDeviceToHost, c->stream));
     SW_CUDA(c, cudaStreamSynchronize(c->stream));
-    c->have_labels = false; c->labels_flat = false; c->sizes_t = ~0ull;
+    c->have_labels = false; c->labels_flat = false; c->sizes_t = ~0ull; c->counts_t = ~0ull;
     if (bad) { c->have_spins = false; return fail(c, SW_ERR_INVALID_ARG, "sw_set_state_packed: spin value >= q"); }
     c->t = t; c->have_spins = true;
     return SW_OK;

@@ -431,6 +431,26 @@ def test_sweep_measure_mask_and_series():
     assert np.array_equal(many.sweep_measure(5000)[::97], ref.sweep_measure(5000)[::97])
 
 
+@pytest.mark.parametrize("flags", [0, sw.FLAG_LAZY_LABELS, sw.FLAG_NO_CLUSTER_PATH])
+@pytest.mark.parametrize("L", [320, 128])
+def test_cluster_count_after_a_series_that_did_not_count(L, flags):
+    """sw_sweep_measure_ex without SW_OBS_CLUSTERS / SW_OBS_LARGEST runs flip kernels that do not count roots; a later
+    sw_measure must not take the per-tile counts of an older sweep (or of no sweep at all) for those of the last one."""
+    q, K = 2, wl.k_critical(2)
+    gpu, cpu = SwendsenWang(L, q, K, 11, flags=flags), Oracle(L, q, K, 11)
+    gpu.init("random"); cpu.init("random")
+    gpu.sweep_measure(3, sw.OBS_ENERGY | sw.OBS_MAG); cpu.sweep(3)       # no sweep of this context has counted yet
+    assert gpu.measure() == cpu.measure()
+    gpu.sweep(2); cpu.sweep(2)                                           # the last sweep of sw_sweep counts
+    assert gpu.measure() == cpu.measure()
+    gpu.sweep_measure(2, sw.OBS_ENERGY); cpu.sweep(2)                    # stale counts of two sweeps ago are in place now
+    assert gpu.measure(energy=False, mag=False, largest=False)["n_clusters"] == cpu.measure()["n_clusters"]
+    assert gpu.measure_clusters()["n_clusters"] == cpu.measure()["n_clusters"]
+    assert gpu.measure() == cpu.measure()
+    assert np.array_equal(gpu.get_labels(), cpu.get_labels()) and np.array_equal(gpu.get_spins(), cpu.get_spins())
+    gpu.close(); cpu.close()
+
+
 def pack_spins(spins, bits):
     """Reference packing in numpy: site i in bits [bits (i % per), ...) of byte i // per."""
     per = 8 // bits
