@@ -208,7 +208,10 @@ const char *sw_version(void);
  * host arrays in the layout of the whole lattice (site i = y*L + x).
  * L % (64 gx) == 0 and L % (64 gy) == 0, gx*gy <= 64, 64 <= L <= 65536; devices that differ must have peer access
  * (NVLink): the bond kernel reads its neighbours' boundary spins and the inter-piece merge hooks roots with
- * system-scope atomicMin directly in the owner's memory.  Device memory is owned by the library.                  */
+ * system-scope atomicMin directly in the owner's memory, so the link must support native atomics
+ * (cudaDevP2PAttrNativeAtomicSupported; PCIe-only peer access does not): otherwise SW_ERR_CUDA, and
+ * sw_super_last_error(NULL) gives the reason of the calling thread's last failed creation.
+ * Device memory is owned by the library.                                                                          */
 typedef struct sw_super sw_super;
 int  sw_create_super(sw_super **out, uint32_t L, uint32_t q, double K, uint64_t seed,
                      uint32_t gx, uint32_t gy, const int *devices /* [gx*gy] or NULL */);
@@ -250,6 +253,11 @@ int  sw_create_super_rank(sw_super **out, uint32_t L, uint32_t q, double K, uint
                           uint32_t gx, uint32_t gy, uint32_t my_piece);
 int  sw_super_ipc_export(sw_super *s, void *handle_out /* host [SW_IPC_HANDLE_BYTES] */);
 int  sw_super_ipc_import(sw_super *s, uint32_t piece, const void *handle /* host [SW_IPC_HANDLE_BYTES] */);
+/* Tear-down of a rank context, first half: waits for the local stream and unmaps every imported piece.  CUDA IPC requires
+ * that an exported allocation is freed only after every importer has closed it, so the ranks call this, THEN pass a barrier
+ * of the process group, THEN call sw_super_destroy (which frees the local piece).  Afterwards the context accepts
+ * sw_super_destroy only (phases and measurements return SW_ERR_STATE).                                                   */
+int  sw_super_ipc_close_all(sw_super *s);
 int  sw_super_phase(sw_super *s, int phase /* 0, 1, 2; phase 2 advances the sweep counter */);
 int  sw_super_measure_phase(sw_super *s, int phase, uint32_t what /* SW_OBS_* */, uint64_t *part /* host [3+q], phase 2 */);
 

@@ -33,7 +33,7 @@ SYMBOLS = [
     "sw_create_super", "sw_super_destroy", "sw_super_init", "sw_super_set_state", "sw_super_sweep", "sw_super_measure",
     "sw_super_get_spins", "sw_super_get_labels", "sw_super_get_bonds", "sw_super_get_time", "sw_super_synchronize",
     "sw_super_get_stats", "sw_super_last_error",
-    "sw_create_super_rank", "sw_super_ipc_export", "sw_super_ipc_import", "sw_super_phase", "sw_super_measure_phase",
+    "sw_create_super_rank", "sw_super_ipc_export", "sw_super_ipc_import", "sw_super_ipc_close_all", "sw_super_phase", "sw_super_measure_phase",
     "sw_xy_create", "sw_xy_destroy", "sw_xy_init", "sw_xy_set_state", "sw_xy_sweep", "sw_xy_measure", "sw_xy_get_spins",
     "sw_xy_get_labels", "sw_xy_get_bonds", "sw_xy_get_reflection", "sw_xy_get_time", "sw_xy_last_error",
     "sw_cluster_stats_static", "sw_static_max_sites", "sw_static_last_error",
@@ -116,6 +116,7 @@ def lib():
     l.sw_super_synchronize.argtypes = [vp]
     l.sw_super_get_stats.argtypes = [vp, C.POINTER(SuperStats)]
     l.sw_super_last_error.argtypes = [vp]; l.sw_super_last_error.restype = C.c_char_p
+    l.sw_super_ipc_close_all.argtypes = [vp]
     dp = C.POINTER(C.c_double)
     l.sw_xy_create.argtypes = [C.POINTER(vp), C.c_uint32, C.c_double, C.c_uint64]
     l.sw_xy_destroy.argtypes = [vp]; l.sw_xy_destroy.restype = None

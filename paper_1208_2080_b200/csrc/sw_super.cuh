@@ -360,14 +360,27 @@ void refresh_geo(sw_super *s)
     }
 }
 
+// why the last sw_create_super / sw_create_super_rank of this thread failed (there is no context to hold the text then)
+thread_local const char *g_create_err = "";
+
+// rank mode: unmap the pieces of the other processes (their pointers are dead afterwards)
+void close_imported(sw_super *s)
+{
+    for (auto &p : s->pieces) {
+        if (p.local || !p.ipc_base) continue;
+        cudaIpcCloseMemHandle(p.ipc_base);
+        p.ipc_base = nullptr;
+        p.ws = nullptr; p.spins = nullptr; p.labels = nullptr; p.edges = nullptr; p.sizes = nullptr;
+    }
+}
+
 void destroy_pieces(sw_super *s)
 {
     DevSwitch sw_;
+    for (auto &p : s->pieces) if (p.local && p.stream) { sw_.to(p.device); cudaStreamSynchronize(p.stream); }   // nothing of mine still reads a peer
+    close_imported(s);
     for (auto &p : s->pieces) {
-        if (!p.local) {
-            if (p.ipc_base) cudaIpcCloseMemHandle(p.ipc_base);
-            continue;
-        }
+        if (!p.local) continue;
         sw_.to(p.device);
         if (p.stream) cudaStreamSynchronize(p.stream);
         if (p.ws) cudaFree(p.ws);
@@ -465,6 +478,7 @@ static int create_super_common(sw_super **out, uint32_t L, uint32_t q, double K,
 {
     if (!out) return SW_ERR_INVALID_ARG;
     *out = nullptr;
+    g_create_err = "";
     uint64_t T = 0;
     if (L < 64 || L > 65536 || q < 2 || q > 255 || !swh::host_threshold(K, &T)) return SW_ERR_INVALID_ARG;
     if (gx < 1 || gy < 1 || gx * gy > (uint32_t)sw::kMaxPieces || L % (gx * sw::kTile) || L % (gy * sw::kTile)) return SW_ERR_INVALID_ARG;
@@ -503,9 +517,17 @@ static int create_super_common(sw_super **out, uint32_t L, uint32_t q, double K,
         for (uint32_t b = 0; b < n && rc == SW_OK; ++b) {
             const int da = s->pieces[a].device, db = s->pieces[b].device;
             if (da == db) continue;
-            int can = 0;
+            int can = 0, native_atomics = 0;
             cudaDeviceCanAccessPeer(&can, da, db);
-            if (!can) { rc = SW_ERR_CUDA; break; }
+            if (!can) { g_create_err = "sw_create_super: two of the devices have no peer access to each other"; rc = SW_ERR_CUDA; break; }
+            // stage 2 and the size count hook roots with atomicMin_system / atomicAdd_system in the owner's memory: over a link
+            // without native atomics (PCIe-only P2P) those are not atomic and labels or sizes would be silently wrong
+            if (cudaDeviceGetP2PAttribute(&native_atomics, cudaDevP2PAttrNativeAtomicSupported, da, db) != cudaSuccess) { cudaGetLastError(); native_atomics = 0; }
+            if (!native_atomics) {
+                g_create_err = "sw_create_super: the link between two of the devices has no native atomics (cudaDevP2PAttrNativeAtomicSupported = 0; "
+                               "NVLink is needed): the inter-piece union-find cannot run over it";
+                rc = SW_ERR_CUDA; break;
+            }
             sw_.to(da);
             const cudaError_t e = cudaDeviceEnablePeerAccess(db, 0);
             if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) rc = SW_ERR_CUDA;
@@ -763,6 +785,18 @@ int sw_super_get_stats(sw_super *s, sw_super_stats *out)
     return SW_OK;
 }
 
-const char *sw_super_last_error(const sw_super *s) { return s ? s->err.c_str() : "null context"; }
+const char *sw_super_last_error(const sw_super *s) { return s ? s->err.c_str() : g_create_err; }
+
+int sw_super_ipc_close_all(sw_super *s)
+{
+    if (!s || s->rank_piece < 0) return sfail(s, SW_ERR_INVALID_ARG, "sw_super_ipc_close_all: not a rank context");
+    DevSwitch sw_;
+    Piece &mine = s->pieces[s->rank_piece];
+    sw_.to(mine.device);
+    SS_CUDA(s, cudaStreamSynchronize(mine.stream));
+    close_imported(s);
+    s->have_spins = false;              // no phase can run any more: sw_super_phase refuses a context with a piece missing
+    return SW_OK;
+}
 
 }  // extern "C"

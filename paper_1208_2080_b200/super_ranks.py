@@ -75,6 +75,11 @@ class LibBackend:
         self._chk(fn(self._h, out.ctypes.data), f"sw_super_get_{what}")
         return out
 
+    def close_imported(self):
+        """Unmap the other ranks' pieces (sw_super_ipc_close_all); the context can only be closed afterwards."""
+        if self._h:
+            self._chk(sw.lib().sw_super_ipc_close_all(self._h), "sw_super_ipc_close_all")
+
     def close(self):
         if self._h:
             sw.lib().sw_super_destroy(self._h)
@@ -112,7 +117,20 @@ class SuperLatticeRanks:
         self._step()
 
     def set_state(self, spins, t):
-        self.backend.set_state(spins, t)
+        """Every rank loads its own piece of `spins`.  If any rank's piece is refused (a spin >= q), EVERY rank raises:
+        the ranks agree on the outcome before the barrier, so no rank is left waiting for one that has already given up."""
+        torch, dist = self._torch, self._dist
+        err = None
+        try:
+            self.backend.set_state(spins, t)
+        except Exception as e:                               # noqa: BLE001 -- reported below, on every rank
+            err = e
+        failed = torch.tensor([0 if err is None else 1], dtype=torch.int32)
+        dist.all_reduce(failed, op=dist.ReduceOp.SUM)
+        if int(failed.item()):
+            if err is not None:
+                raise err
+            raise sw.SwError(sw.ERR_INVALID_ARG, "sw_super_set_state", f"refused on {int(failed.item())} other rank(s)")
         self._step()
 
     def sweep(self, n=1):
@@ -147,5 +165,9 @@ class SuperLatticeRanks:
         return t.numpy().astype(local.dtype)
 
     def close(self):
-        self._dist.barrier()
+        """Tear-down in three steps: every rank unmaps the pieces it imported, THEN (barrier) every rank frees its own.
+        Freeing an exported piece while another process still has it mapped is undefined behaviour in CUDA IPC."""
+        self._dist.barrier()                                 # nobody is still inside a phase
+        self.backend.close_imported()
+        self._dist.barrier()                                 # nobody has my piece mapped any more
         self.backend.close()

@@ -8,6 +8,7 @@ import os
 import socket
 import time
 
+import numpy as np
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
@@ -50,8 +51,16 @@ class RecordingBackend:
         # energy, n_clusters, largest, mag[q]
         return [10 * (self.rank + 1), 3 + self.rank, 100 + 7 * self.rank] + [self.rank + s for s in range(self.q)]
 
+    def set_state(self, spins, t):
+        if self.rank == 1 and int(np.max(spins)) >= self.q:
+            raise ValueError("spin value >= q on rank 1")
+        self._rec(("set_state", int(t)))
+
+    def close_imported(self):
+        self._rec("close_imported")
+
     def close(self):
-        pass
+        self._rec("close")
 
 
 def _worker(rank, world, port, gx, gy, log, out):
@@ -64,6 +73,14 @@ def _worker(rank, world, port, gx, gy, log, out):
         sim.init("random")
         sim.sweep(3)
         out[rank] = (sim.measure(), sorted(be.imported))
+        # a state that only rank 1 refuses: every rank must raise (and none may hang in the barrier that follows)
+        L = 128 * gx
+        try:
+            sim.set_state(np.full(L * L, 3, dtype=np.uint8), 5)
+            out[("set_state", rank)] = "accepted"
+        except Exception as e:                               # noqa: BLE001
+            out[("set_state", rank)] = type(e).__name__
+        sim.set_state(np.zeros(L * L, dtype=np.uint8), 5)    # the ranks are still in step afterwards
         sim.close()
     finally:
         dist.destroy_process_group()
@@ -81,6 +98,7 @@ def check(gx, gy):
     world = gx * gy
     log, out = _run(gx, gy)
     for rank in range(world):
+        assert out[("set_state", rank)] == ("ValueError" if rank == 1 else "SwError")
         m, imported = out[rank]
         assert imported == [r for r in range(world) if r != rank]
         assert m["energy_bonds"] == 10 * sum(r + 1 for r in range(world))
@@ -89,7 +107,13 @@ def check(gx, gy):
         assert m["mag_counts"] == [sum(r + s for r in range(world)) for s in range(3)]
     # lock step: the steps appear in the same order on every rank, and step k ends everywhere before step k + 1 begins anywhere
     steps = [w for (_, r, kind, w) in log if r == 0 and kind == "begin"]
-    assert steps == [("init", "random")] + [("phase", k) for _ in range(3) for k in (0, 1, 2)] + [("measure", k) for k in (0, 1, 2)]
+    in_step = [("init", "random")] + [("phase", k) for _ in range(3) for k in (0, 1, 2)] + [("measure", k) for k in (0, 1, 2)]
+    # (rank 0's own piece was accepted both times; the first time it raised all the same, because rank 1 refused)
+    assert steps == in_step + [("set_state", 5), ("set_state", 5), "close_imported", "close"]
+    steps = in_step
+    # tear-down: every rank has unmapped its imports before any rank frees its piece
+    assert max(t for (t, r, kind, w) in log if kind == "end" and w == "close_imported") <= \
+        min(t for (t, r, kind, w) in log if kind == "begin" and w == "close")
     for i in range(len(steps) - 1):
         ends = [t for (t, r, kind, w) in log if kind == "end" and w == steps[i]]
         later = [j for j, (t, r, kind, w) in enumerate(log) if kind == "begin" and w == steps[i + 1]]
