@@ -356,7 +356,8 @@ class SuperLattice:
         rc = lib().sw_create_super(C.byref(self._h), self.L, self.q, self.K, self.seed, self.gx, self.gy, dev)
         if rc != OK:
             self._h = C.c_void_p()
-            raise SwError(rc, "sw_create_super")
+            why = lib().sw_super_last_error(None)             # (no context to ask: the reason of this thread's last failed creation)
+            raise SwError(rc, "sw_create_super", why.decode() if why else "")
 
     def close(self):
         if self._h:

@@ -135,3 +135,32 @@ def test_config4_size_q10_in_2x2_pieces_one_transition():
     cpu.set_state(sup.get_spins(), sup.get_time())
     sup.sweep(1); cpu.sweep(1)
     compare(sup, cpu, "(c4 below, 2x2 pieces, t = 40)")
+
+
+def _n_devices():
+    import torch
+    return torch.cuda.device_count() if torch.cuda.is_available() else 0
+
+
+@pytest.mark.parametrize("gx,gy,devices", [(2, 1, [0, 1]), (2, 2, [0, 1, 1, 0]), (1, 2, [1, 0])])
+def test_pieces_on_two_devices_peer_path(gx, gy, devices):
+    """The path the paper is about: pieces on DIFFERENT GPUs, neighbours' boundary spins read over the
+    link, roots hooked with system-scope atomics in the owner's memory.  Needs two devices with peer access and native
+    atomics between them (NVLink); skipped on a one-GPU box, so it runs the first time such hardware is there."""
+    if _n_devices() < 2:
+        pytest.skip("needs two CUDA devices (the peer / NVLink path)")
+    L, q = 512, 2
+    K = wl.k_critical(q)
+    try:
+        gpu = SuperLattice(L, q, K, 5, gx, gy, devices=devices)
+    except sw.SwError as e:                                   # peer access or native atomics missing: say so, do not fail
+        pytest.skip(f"sw_create_super refused these devices: {sw.lib().sw_super_last_error(None).decode()} ({e})")
+    cpu = Oracle(L, q, K, 5)
+    gpu.init("random"); cpu.init("random")
+    assert gpu.stats()["devices"] == 2
+    for k in range(4):
+        gpu.sweep(1); cpu.sweep(1)
+        compare(gpu, cpu, f"({gx}x{gy} on devices {devices}, sweep {k})")
+    gpu.sweep(3); cpu.sweep(3)
+    compare(gpu, cpu, f"({gx}x{gy} on devices {devices}, after 3 more)")
+    assert gpu.stats()["inter_links"] > 0
