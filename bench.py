@@ -63,15 +63,18 @@ ALU_OPS_PER_SITE_BONDS = 0.5 * 40 + 2 + 2
 ALU_OPS_PER_CLUSTER = 40
 B200_SMS, B200_LANES_PER_SM = 148, 128
 
-# the other BASELINE.json configs, measured briefly in the same run: (name, warm-up sweeps, timed sweeps, observables the
-# config asks for every sweep -- None = update only)
+# the other BASELINE.json configs, measured in the same run: (name, warm-up sweeps, timed sweeps, observables the config
+# asks for every sweep -- None = update only, start -- None = the config's own).  Warm-up + timed = the config's own
+# number of sweeps: the timed half is the second half of the run the config describes, and the record carries the ratio
+# of the first to the second half of its per-sweep series (1.00 = flat, i.e. no transient left in the number).
+# q = 4 starts ordered: from a random start it is still 3 % off after 100 sweeps at L = 1024.
 OTHER_CONFIGS = [
-    ("c1_L256_q2", 20, 200, "all"),
-    ("c2_L4096_q2", 40, 40, None),
-    ("c3_L8192_q3", 30, 20, "energy+mag"),
-    ("c3_L8192_q4", 30, 20, "energy+mag"),
-    ("c4_L16384_q10_above", 30, 20, "clusters+largest"),
-    ("c4_L16384_q10_below", 30, 20, "clusters+largest"),
+    ("c1_L256_q2", 100, 100, "all", None),
+    ("c2_L4096_q2", 500, 500, None, None),
+    ("c3_L8192_q3", 250, 250, "energy+mag", None),
+    ("c3_L8192_q4", 250, 250, "energy+mag", "ordered"),
+    ("c4_L16384_q10_above", 100, 100, "clusters+largest", None),
+    ("c4_L16384_q10_below", 100, 100, "clusters+largest", None),
 ]
 
 
@@ -244,9 +247,11 @@ def time_cpu_baseline(args, equilibrated):
 
 # ------------------------------------------------------------------------------------------------ GPU arm
 
-def measure_config(name, warm, steps, what, torch, SwendsenWang, sw):
-    """Brief measurement of one of the other BASELINE.json configs: update-only, and with the observables it asks for."""
-    c = wl.CONFIGS[name]
+def measure_config(name, warm, steps, what, start, torch, SwendsenWang, sw):
+    """One of the other BASELINE.json configs: update-only, and with the observables it asks for."""
+    c = dict(wl.CONFIGS[name])
+    if start:
+        c["start"] = start
     L, N = c["L"], c["L"] ** 2
     sim = SwendsenWang(L, c["q"], c["K"], c["seed"])
     sim.init(c["start"])
@@ -256,8 +261,14 @@ def measure_config(name, warm, steps, what, torch, SwendsenWang, sw):
     e0.record(); sim.sweep(steps); e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps
-    rec = {"L": L, "q": c["q"], "start": c["start"], "warmup": warm, "steps": steps,
+    rec = {"L": L, "q": c["q"], "start": c["start"], "warmup": warm, "steps": steps, "config_sweeps": c["sweeps"],
            "flips_per_ns": N / (ms * 1e-3) / 1e9, "ms_per_sweep": ms, "path": sim.stats()["path_name"]}
+    if sim.stats()["path"] == 1:                                    # per-sweep series (a second pass, events around every kernel)
+        sim.profile_begin(); sim.sweep(steps); sim.profile_end()
+        ser = sim.last_series
+        if len(ser) >= 4:
+            h = len(ser) // 2
+            rec["series_first_half_over_second_half"] = (sum(ser[:h]) / h) / (sum(ser[h:]) / (len(ser) - h))
     if what:
         mask = {"all": sw.OBS_ALL, "energy+mag": sw.OBS_ENERGY | sw.OBS_MAG, "clusters+largest": sw.OBS_CLUSTERS | sw.OBS_LARGEST}[what]
         sim.sweep_measure(2, mask)                                  # warm (first call allocates / sizes scratch)
@@ -343,6 +354,29 @@ def run_gpu(args):
     e1.record()
     torch.cuda.synchronize()
     value_meas = N * m_steps / (e0.elapsed_time(e1) * 1e-3) / 1e9
+    # the same with ALL FOUR outputs of sw_measure (largest_cluster too: a 4 N-byte size counter per site, 16 GiB at
+    # L = 65536, allocated by the library on first use), once as sweep + sw_measure per step, once as ONE
+    # sw_sweep_measure call (sizes counted inside the tile / flip kernels, no per-site counting pass)
+    value_meas_all = value_series_all = None
+    if world == 1 and not args.lazy and not args.label_equivalence:
+        a_steps = max(1, min(args.steps, 5))
+        sim.measure()                                          # (untimed: allocates the size counters)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(a_steps):
+            sim.sweep(1)
+            obs_all = sim.measure()
+        e1.record()
+        torch.cuda.synchronize()
+        value_meas_all = N * a_steps / (e0.elapsed_time(e1) * 1e-3) / 1e9
+        sim.sweep_measure(1)                                   # (untimed: first use of the counting instantiations)
+        torch.cuda.synchronize()
+        e0.record()
+        rows_all = sim.sweep_measure(a_steps)
+        e1.record()
+        torch.cuda.synchronize()
+        value_series_all = N * a_steps / (e0.elapsed_time(e1) * 1e-3) / 1e9
+        assert int(rows_all[-1, 2]) >= 1 and int(rows_all[-1, 1]) >= 1
 
     # ---- end to end through the C ABI with HOST buffers: H2D of the state, one sweep, D2H of the new state, every step.
     # The state crosses PCIe in the library's packed form (sw_set_state_packed / sw_get_spins_packed: 1 bit per spin at
@@ -440,9 +474,9 @@ def run_gpu(args):
         sim.close()
         torch.cuda.empty_cache()
         other = {}
-        for name, warm, steps, what in OTHER_CONFIGS:
+        for name, warm, steps, what, start in OTHER_CONFIGS:
             try:
-                other[name] = measure_config(name, warm, steps, what, torch, SwendsenWang, sw)
+                other[name] = measure_config(name, warm, steps, what, start, torch, SwendsenWang, sw)
             except Exception as e:                                   # a failed side measurement must not lose the headline line
                 other[name] = {"error": repr(e)}
 
@@ -470,6 +504,23 @@ def run_gpu(args):
                 "what": "wall clock around 20 sweeps + synchronize, all four pieces on this GPU; NVLink unmeasured"}
         except Exception as e:
             other["super_2x2_L16384_q2_one_device"] = {"error": repr(e)}
+
+    # ---- the extension the paper names: embedded-cluster sweeps of the XY model.
+    # It runs on the any-L generic kernels (global union-find), untuned: the number says where it stands, not what the
+    # hardware allows.  Bytes per site per sweep as built: spins R 16 + W 16 (double x, y), labels 4 x 3 passes, bond bits 0.5.
+    if other is not None:
+        try:
+            from paper_1208_2080_b200.binding import XYModel
+            for Lxy in (4096, 8192):
+                xy = XYModel(Lxy, 1.12, 1)                         # K near the Kosterlitz-Thouless point: clusters of all sizes
+                xy.init("random"); xy.sweep(10); xy.measure()
+                t0 = time.perf_counter(); xy.sweep(10); m_xy = xy.measure(); dt = time.perf_counter() - t0
+                xy.close()
+                other[f"xy_L{Lxy}"] = {"flips_per_ns": Lxy * Lxy * 10 / dt / 1e9, "ms_per_sweep": dt / 10 * 1e3, "K": 1.12, "warmup": 10, "steps": 10,
+                                       "bytes_per_site_as_built": 44.5, "n_clusters": m_xy["n_clusters"],
+                                       "what": "wall clock around sw_xy_sweep(10) + one sw_xy_measure (synchronises); generic kernels, untuned"}
+        except Exception as e:
+            other["xy"] = {"error": repr(e)}
 
     # ---- the oracle on this box's host cores (reported baseline, rank 0, N = 1 only), on equilibrated lattices
     cpu_baseline = None
@@ -507,7 +558,11 @@ def run_gpu(args):
                         "what": "SURVEY.md sec. 8(d): 14.5 + 24/T_tile bytes per site per sweep over the measured copy bandwidth"},
         "time_series": time_series,
         "update_plus_measurement": {"value": value_meas, "unit": UNIT, "steps": m_steps,
-                                    "what": "sw_sweep(1) + sw_measure(energy, magnetisation, n_clusters) per step"},
+                                    "what": "sw_sweep(1) + sw_measure(energy, magnetisation, n_clusters) per step: THREE of the four observables",
+                                    "all_four_observables": None if value_meas_all is None else {
+                                        "sweep_then_sw_measure": value_meas_all, "sw_sweep_measure_ex_OBS_ALL": value_series_all, "unit": UNIT,
+                                        "steps": a_steps, "what": "the same with largest_cluster as well (all outputs of sw_measure): per-step "
+                                        "sw_sweep(1) + sw_measure, and one sw_sweep_measure(n) call"}},
         "other_configs": other,
         "last_observables": obs,
         "label_equivalence_rounds_per_sweep": (stats["le_rounds_total"] / stats["sweeps"]) if args.label_equivalence else None,
@@ -521,6 +576,79 @@ def run_gpu(args):
 
 
 # ------------------------------------------------------------------------------------------------ control plane only (tests)
+
+def run_super(args):
+    """`--super GXxGY`: ONE lattice cut into gx x gy pieces, the axis the paper's Table 1 scales along.
+    With N = gx*gy ranks (torchrun) every rank owns one piece on its own GPU and reaches the others through CUDA IPC
+    peer pointers (NVLink); with one rank all the pieces sit on this GPU.  value = L^2 * sweeps / time of the ONE lattice
+    (strong scaling).  The phases of a sweep are ordered by the host (events in one process, a process-group barrier
+    between ranks), so the clock is the wall clock around sweep + synchronize, max over ranks."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_1208_2080_b200.binding import SuperLattice
+    gx, gy = (int(v) for v in args.super.lower().split("x"))
+    rank, local_rank, world = rank_info()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU path")
+    if world not in (1, gx * gy):
+        raise SystemExit(f"bench.py: --super {args.super} needs 1 rank (all pieces on one GPU) or {gx * gy} ranks (one piece each), not {world}")
+    torch.cuda.set_device(local_rank)
+    c = wl.CONFIGS[args.workload]
+    L, q, K, N = c["L"], c["q"], c["K"], c["L"] ** 2
+    if world > 1:
+        from paper_1208_2080_b200.super_ranks import SuperLatticeRanks
+        dist.init_process_group("gloo")          # control plane only (64-byte handles, barriers); the data path is peer memory
+        sim = SuperLatticeRanks(L, q, K, c["seed"], gx, gy)
+    else:
+        sim = SuperLattice(L, q, K, c["seed"], gx, gy)
+    sync = (lambda: None) if world > 1 else sim.synchronize     # (a rank-mode sweep ends with synchronize + barrier already)
+    sim.init(c["start"])
+    sim.sweep(args.warmup); sync()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    if world > 1:
+        dist.barrier()
+    wall0 = time.time()
+    t0 = time.perf_counter()
+    sim.sweep(args.steps); sync()
+    dt = time.perf_counter() - t0
+    wall1 = time.time()
+    clocks = sampler.stop(wall0, wall1) if rank == 0 else None
+    st = sim.backend.stats() if world > 1 else sim.stats()
+    sums = torch.tensor([st["inter_links"], st["inter_hops"], st["inter_retries"], st["resolved_links"], st["kernel_launches"]], dtype=torch.int64)
+    slowest = torch.tensor([dt], dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(slowest, op=dist.ReduceOp.MAX)
+        dist.all_reduce(sums, op=dist.ReduceOp.SUM)               # every rank counts its own piece's share
+    dt = float(slowest.item())
+    sweeps = st["sweeps"]
+    obs = sim.measure()
+    if rank == 0:
+        value = N * args.steps / dt / 1e9
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": (value / PAPER_FLIPS_PER_NS) if args.workload == wl.HEADLINE else None,
+            "dtype": "u32", "data": "synthetic",
+            "config": {"workload": args.workload, "L": L, "q": q, "K": K, "start": c["start"], "seed": c["seed"],
+                       "decomposition": f"{gx}x{gy} pieces of {L // gx}x{L // gy}", "parallelism": f"{world} GPU(s), {gx * gy // world} piece(s) each",
+                       "timing": "wall clock around sw_super_sweep + synchronize, max over ranks (host-ordered phases)",
+                       "l2": "working set >> 126 MB L2, no flush needed" if N * 6 > (126 << 20) * 4 else "lattice fits L2"},
+            "clocks": clocks, "gpu_launches": int(sums[4]) * args.steps // max(1, sweeps),
+            "super": {"inter_piece_links_per_sweep": int(sums[0]) / sweeps, "inter_piece_label_loads_per_sweep": int(sums[1]) / sweeps,
+                      "lost_hook_races_per_sweep": int(sums[2]) / sweeps, "resolved_links_per_sweep": int(sums[3]) / sweeps,
+                      "boundary_sites_per_piece": st["boundary_sites_per_piece"],
+                      "what": "label loads of stage 2 + resolve = the traffic that crosses NVLink when the pieces sit on different GPUs "
+                              "(4 bytes each; the paper exchanges 4 N_x labels per GPU per round, PAPER.md:68)"},
+            "last_observables": obs}))
+    sim.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
 
 def run_control_plane_only(args):
     """Test hook (tests/test_bench_ranks.py): the rank plumbing of the N > 1 path on CPU -- gloo rendezvous, replica seeds,
@@ -560,11 +688,13 @@ def main():
     ap.add_argument("--lazy", action="store_true", help="SW_FLAG_LAZY_LABELS: canonical labels flattened on demand only")
     ap.add_argument("--label-equivalence", action="store_true",
                     help="SW_FLAG_LABEL_EQUIVALENCE: the paper's scan + analysis labeling (comparison variant, not the product path)")
-    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true")
     ap.add_argument("--cpu-baseline-sweeps", type=int, default=20)
     ap.add_argument("--reference-L", type=int, default=2048)
+    ap.add_argument("--super", default=None, metavar="GXxGY",
+                    help="the super-lattice decomposition of ONE lattice (PAPER.md:62-84): gx*gy ranks with one piece per GPU, or 1 rank")
     ap.add_argument("--control-plane-only", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
     if args.gpus < 1:
@@ -583,6 +713,8 @@ def main():
     args.warmup = 60 if args.warmup is None else args.warmup
     if args.control_plane_only:
         return run_control_plane_only(args)
+    if args.super:
+        return run_super(args)
     return run_gpu(args)
 
 

@@ -75,6 +75,12 @@ class LibBackend:
         self._chk(fn(self._h, out.ctypes.data), f"sw_super_get_{what}")
         return out
 
+    def stats(self):
+        """sw_super_get_stats of this rank's context (the counters cover the local piece's share of the work)."""
+        st = sw.SuperStats()
+        self._chk(sw.lib().sw_super_get_stats(self._h, C.byref(st)), "sw_super_get_stats")
+        return {f: int(getattr(st, f)) for f, _ in sw.SuperStats._fields_}
+
     def close_imported(self):
         """Unmap the other ranks' pieces (sw_super_ipc_close_all); the context can only be closed afterwards."""
         if self._h:
