@@ -27,7 +27,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     newest = max(os.path.getmtime(os.path.join(CSRC, d)) for d in DEPS)
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
-    cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+    extra = os.environ.get("SW_NVCC_EXTRA", "").split()      # e.g. SW_NVCC_EXTRA=-DSW_FLIP_TMA=1 (an experiment recorded in DESIGN.md sec. 6)
+    cmd = [nvcc_path()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
           ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.run(cmd, check=True, cwd=CSRC)
     return LIB

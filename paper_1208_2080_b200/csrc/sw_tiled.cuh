@@ -251,13 +251,46 @@ struct FlipShared {
 // clusters and were dealt with there); each adds its size to sizes[canonical root] -- one global atomic per such
 // component, nothing per site -- so that afterwards sizes[] (all zero before) holds the sizes of the clusters that
 // cross a tile border at their canonical roots.
-template <bool kLabels, bool kSpins, bool kCount, bool kStats, bool kSuper, int NT, class Bar, bool kSizes = false>
+//
+// kTma (experiment, SW_FLIP_TMA; k_tile_flip only): the label rows of the tile move by TMA bulk copies (cp.async.bulk,
+// SASS UBLKCP) instead of 16-byte cp.async per thread.  A tile row is 256 contiguous bytes in global AND in S.root, so
+// each warp fetches its own kRows rows with one bulk copy per row (lanes 0 .. kRows-1 issue one each) that complete on
+// the warp's own mbarrier -- no CTA barrier, the warp waits for its own rows only, like cp.async.wait_all did.
+// kTma == 2: the canonical labels leave the same way: phase C writes them over the warp's own rows of S.root (a root's
+// entry already IS its label; the other entries are read by their owner only, before it overwrites them) and one
+// bulk store per row sends them out.  Measured numbers: DESIGN.md sec. 6.
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
+                 :: "r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_load(uint32_t dst_smem, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(dst_smem), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void bulk_store(void *dst, uint32_t src_smem, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" :: "l"(dst), "r"(src_smem), "r"(bytes) : "memory");
+}
+
+template <bool kLabels, bool kSpins, bool kCount, bool kStats, bool kSuper, int NT, class Bar, bool kSizes = false, int kTma = 0>
 __device__ __forceinline__ void
 tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t *labels, const uint16_t *rootbits, uint8_t *spins,
                const Params &P, const uint32_t (&pk_t)[3], const uint32_t (&pk_n)[3], const Dom &dom,
                uint32_t *tile_clusters, uint2 *next_draws, PassCounters *counters, uint32_t *sizes = nullptr,
-               const uint32_t *btab = nullptr)
+               const uint32_t *btab = nullptr, unsigned long long *mbar = nullptr)
 {
+    static_assert(kTma == 0 || !kSuper, "the bulk-copy variant is written for the single lattice");
     constexpr int kAcc = FlipShared<NT>::kAcc, kRows = FlipShared<NT>::kRows;
     const uint32_t tid = threadIdx.x;
     const uint32_t lane = tid & 31u, warp = tid >> 5;
@@ -287,11 +320,23 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
     // while they are in flight): a root's entry is where its chase starts (and is replaced by the canonical root
     // below), every other site's entry keeps the tile-local id of its root until phase C reads it back -- nothing
     // per site has to stay in registers across the draws and the chases.
+    uint32_t bar = 0;
+    if (kTma) {
+        bar = (uint32_t)__cvta_generic_to_shared(mbar + warp);
+        if (lane == 0) { mbar_init(bar, 1); mbar_expect_tx(bar, kRows * kTile * 4); }
+        __syncwarp();
+        if (lane < (uint32_t)kRows) {                          // one 256-byte row each
+            const uint32_t row = warp * kRows + lane;
+            bulk_load((uint32_t)__cvta_generic_to_shared(&S.root[row << 6]), labels + origin + row * W, kTile * 4, bar);
+        }
+    }
 #pragma unroll
     for (int k = 0; k < kAcc; ++k) {
         const uint32_t o = a00 + 2 * k * W, id0 = ((yk0 + 2 * k) << 6) + x4;
-        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&S.root[id0]);
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(dst), "l"(labels + o) : "memory");
+        if (!kTma) {
+            const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&S.root[id0]);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(dst), "l"(labels + o) : "memory");
+        }
         rq[k] = rootbits[o >> 4];
     }
     // while those loads are on their way: the bond draws of the NEXT sweep for this tile (pure arithmetic, see above)
@@ -301,7 +346,7 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
     }
 #pragma unroll
     for (int k = 0; k < kAcc; ++k) work |= ((rq[k] >> (x4 & 12u)) & 15u) << (4 * k);
-    asm volatile("cp.async.wait_all;" ::: "memory");
+    if (kTma) mbar_wait(bar, 0); else asm volatile("cp.async.wait_all;" ::: "memory");
 
     {
         // each warp lists the tile-local roots of its rows (prefix sum over the lanes, no atomics) ...
@@ -370,8 +415,20 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
             if (kSpins) st |= (uint32_t)S.state[id] << (8 * j);
         }
         if (kSpins) *reinterpret_cast<uint32_t *>(spins + o) = st;
-        if (kLabels)
+        if (kLabels && kTma == 2)
+            *reinterpret_cast<uint4 *>(&S.root[((yk0 + 2 * k) << 6) + x4]) = make_uint4(lab[0], lab[1], lab[2], lab[3]);
+        else if (kLabels)
             *reinterpret_cast<uint4 *>(labels + o) = make_uint4(lab[0], lab[1], lab[2], lab[3]);
+    }
+    if (kLabels && kTma == 2) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // my writes to S.root, before the async proxy reads them
+        __syncwarp();
+        if (lane < (uint32_t)kRows) {
+            const uint32_t row = warp * kRows + lane;
+            bulk_store(labels + origin + row * W, (uint32_t)__cvta_generic_to_shared(&S.root[row << 6]), kTile * 4);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory must outlive the read
+        }
     }
     if (kCount) {
         canon = __reduce_add_sync(0xFFFFFFFFu, canon);
@@ -382,14 +439,23 @@ tile_flip_body(FlipShared<NT> &S, const uint32_t tx, const uint32_t ty, uint32_t
 #ifndef SW_FLIP_CTAS
 #define SW_FLIP_CTAS 7
 #endif
+#ifndef SW_FLIP_TMA
+#define SW_FLIP_TMA 0        // 0: 16-byte cp.async per thread (kept: see DESIGN.md sec. 6), 1: TMA bulk loads, 2: bulk loads and stores
+#endif
 template <bool kLabels, bool kSpins, bool kCount, bool kStats = false>
 __global__ void __launch_bounds__(kFlipThreads, SW_FLIP_CTAS)
 k_tile_flip(uint32_t *labels, const uint16_t *__restrict__ rootbits, uint8_t *__restrict__ spins, Params P,
             uint32_t *__restrict__ tile_clusters, uint2 *__restrict__ next_draws, PassCounters *__restrict__ counters = nullptr)
 {
-    __shared__ FlipShared<kFlipThreads> S;
+    __shared__ __align__(128) FlipShared<kFlipThreads> S;
+#if SW_FLIP_TMA
+    __shared__ unsigned long long mbar[kFlipThreads / 32];     // one mbarrier per warp (its own rows)
+    tile_flip_body<kLabels, kSpins, kCount, kStats, false, kFlipThreads, MergeBar, false, SW_FLIP_TMA>(
+        S, blockIdx.x, blockIdx.y, labels, rootbits, spins, P, P.pk_t, P.pk_n, Dom{}, tile_clusters, next_draws, counters, nullptr, nullptr, mbar);
+#else
     tile_flip_body<kLabels, kSpins, kCount, kStats, false, kFlipThreads, MergeBar>(
         S, blockIdx.x, blockIdx.y, labels, rootbits, spins, P, P.pk_t, P.pk_n, Dom{}, tile_clusters, next_draws, counters);   // grid = (tiles_x, tiles_x): no division
+#endif
 }
 
 // the flip of a sweep whose cluster sizes are wanted (sw_sweep_measure with SW_OBS_LARGEST): eager labels, spins, cluster
