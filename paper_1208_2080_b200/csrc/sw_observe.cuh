@@ -155,24 +155,43 @@ k_observe_vec16(const uint8_t *__restrict__ spins, const uint32_t *__restrict__ 
     if (want & 4u) block_add_u64(roots, row + 1, s_scratch);
 }
 
-// sizes[root(i)] += 1, with run-length aggregation over consecutive sites (clusters are spatially
-// coherent, so a thread's 16 sites usually share one or two roots).  Works on a forest too.
+// sizes[root(i)] += 1.  Clusters are spatially coherent, so a thread's 16 consecutive sites usually belong to one or two
+// clusters: it counts them in two private slots (a third label evicts the slot with the smaller count), and at the end of
+// the group the lanes of a warp that hold the same root add their counts up (match_any + reduce) so that ONE lane does the
+// atomic.  At criticality one cluster holds a large fraction of all sites: without the two slots every hole in it cost an
+// atomic on the same address, and without the warp step 2^32 / 16 threads queued up on that one address (420 ms per call at
+// L = 65536; SURVEY.md sec. 8 config 4's largest_cluster through sw_measure).  Works on a forest too.
+__device__ __forceinline__ void warp_add_size(uint32_t *sizes, uint32_t root, uint32_t n)
+{
+    const unsigned here = __activemask();
+    const unsigned has = __ballot_sync(here, n != 0u);
+    if (n) {
+        const unsigned peers = __match_any_sync(has, root);
+        const uint32_t total = __reduce_add_sync(peers, n);
+        if ((threadIdx.x & 31u) == (uint32_t)__ffs(peers) - 1u) atomicAdd(sizes + root, total);
+    }
+}
+
 __global__ void k_cluster_sizes(const uint32_t *__restrict__ labels, uint32_t *sizes, Params P)
 {
     const uint64_t n_groups = (P.N + 15) >> 4;
     const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     for (uint64_t g = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; g < n_groups; g += stride) {
-        uint32_t cur = 0, run = 0;
+        uint32_t ra = 0, na = 0, rb = 0, nb = 0;
         for (uint32_t j = 0; j < 16; ++j) {
             const uint64_t i = (g << 4) + j;
             if (i >= P.N) break;
             uint32_t l = labels[i];
             if (l != (uint32_t)i) l = find_root(labels, l);
-            if (run && l == cur) { ++run; continue; }
-            if (run) atomicAdd(sizes + cur, run);
-            cur = l; run = 1;
+            if (na && l == ra) ++na;
+            else if (nb && l == rb) ++nb;
+            else if (!na) { ra = l; na = 1; }
+            else if (!nb) { rb = l; nb = 1; }
+            else if (na < nb) { atomicAdd(sizes + ra, na); ra = l; na = 1; }
+            else { atomicAdd(sizes + rb, nb); rb = l; nb = 1; }
         }
-        if (run) atomicAdd(sizes + cur, run);
+        warp_add_size(sizes, ra, na);
+        warp_add_size(sizes, rb, nb);
     }
 }
 
